@@ -1,0 +1,138 @@
+"""ctypes front end of the CPU oracle (oracle/gspn_oracle.c).
+
+TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference leg.  Nothing under
+paper_2606_00746_b200/ imports this module and this module imports nothing
+from there.
+
+All functions take and return C-contiguous numpy arrays in the layouts of
+include/gspn.h (x [B,C,H,W]; w3 [D,B,G,3,H,W]; lambda,u [D,B,C,H,W];
+h0/dh0 [D,B,C,max(H,W)]).  dtype float64 selects the truth build, float32 the
+pinned-order diagnostic build.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "gspn_oracle.c")
+_HDR = os.path.join(_HERE, "gspn_oracle_impl.h")
+_LIB = os.path.join(_HERE, "libgspn_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (plain -O2, OpenMP over planes, no FMA contraction)."""
+    stale = (not os.path.exists(_LIB)
+             or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_HDR)))
+    if force or stale:
+        cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared",
+               "-o", _LIB + ".tmp", _SRC, "-lm"]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+        os.replace(_LIB + ".tmp", _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+    return _lib
+
+
+def threads() -> int:
+    return int(_load().gspn_oracle_threads())
+
+
+def set_threads(n: int) -> None:
+    _load().gspn_oracle_set_threads(int(n))
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _prep(a, dt):
+    if a is None:
+        return None
+    a = np.ascontiguousarray(a, dtype=dt)
+    return a
+
+
+def popcount(mask: int) -> int:
+    return bin(mask & 15).count("1")
+
+
+def _check(x, w3, lam, u, G, mask, h0=None):
+    B, C, H, W = x.shape
+    D = popcount(mask)
+    assert w3.shape == (D, B, G, 3, H, W), (w3.shape, (D, B, G, 3, H, W))
+    assert lam.shape == (D, B, C, H, W) and u.shape == (D, B, C, H, W)
+    if h0 is not None:
+        assert h0.shape == (D, B, C, max(H, W))
+    return B, C, H, W, D
+
+
+def fwd(x, w3, lam, u, G: int, mask: int, h0=None, return_h: bool = False):
+    """y = sum_d u_d * scan_d(x)  (Eq. 1, 2, 5, 9).  Returns y or (y, h[D,B,C,H,W])."""
+    dt = np.float32 if x.dtype == np.float32 else np.float64
+    x, w3, lam, u, h0 = (_prep(a, dt) for a in (x, w3, lam, u, h0))
+    B, C, H, W, D = _check(x, w3, lam, u, G, mask, h0)
+    y = np.empty_like(x)
+    hs = np.empty((D, B, C, H, W), dtype=dt) if return_h else None
+    fn = _load().gspn_oracle_fwd_f32 if dt == np.float32 else _load().gspn_oracle_fwd_f64
+    rc = fn(_ptr(x), _ptr(w3), _ptr(lam), _ptr(u), _ptr(h0), _ptr(y), _ptr(hs),
+            B, C, H, W, int(G), ctypes.c_uint(mask))
+    if rc != 0:
+        raise ValueError("gspn_oracle_fwd: invalid arguments")
+    return (y, hs) if return_h else y
+
+
+def bwd(x, w3, lam, u, dy, G: int, mask: int, h0=None):
+    """Adjoint of fwd.  Returns dict(dx, dlambda, du, dw3, dh0)."""
+    dt = np.float32 if x.dtype == np.float32 else np.float64
+    x, w3, lam, u, dy, h0 = (_prep(a, dt) for a in (x, w3, lam, u, dy, h0))
+    B, C, H, W, D = _check(x, w3, lam, u, G, mask, h0)
+    assert dy.shape == x.shape
+    out = dict(dx=np.empty_like(x), dlambda=np.empty_like(lam), du=np.empty_like(u),
+               dw3=np.empty_like(w3), dh0=np.empty((D, B, C, max(H, W)), dtype=dt))
+    fn = _load().gspn_oracle_bwd_f32 if dt == np.float32 else _load().gspn_oracle_bwd_f64
+    rc = fn(_ptr(x), _ptr(w3), _ptr(lam), _ptr(u), _ptr(h0), _ptr(dy), _ptr(out["dx"]),
+            _ptr(out["dlambda"]), _ptr(out["du"]), _ptr(out["dw3"]), _ptr(out["dh0"]),
+            B, C, H, W, int(G), ctypes.c_uint(mask))
+    if rc != 0:
+        raise ValueError("gspn_oracle_bwd: invalid arguments")
+    return out
+
+
+def merge(y_dirs, m=None):
+    """y = sum_q m[q,c] * y_dirs[q]  (m None = ones)."""
+    y_dirs = _prep(y_dirs, np.float64)
+    m = _prep(m, np.float64)
+    D, B, C, H, W = y_dirs.shape
+    y = np.empty((B, C, H, W), dtype=np.float64)
+    rc = _load().gspn_oracle_merge_f64(_ptr(y_dirs), _ptr(m), _ptr(y), D, B, C, H, W)
+    if rc != 0:
+        raise ValueError("gspn_oracle_merge: invalid arguments")
+    return y
+
+
+def fwd_magnitude(x, w3, lam, u, G: int, mask: int, h0=None):
+    """A >= |y| elementwise: the same recurrence on |x|, |lambda|, |u|, |w3|, |h0|.
+
+    A_i is the sum of the absolute values of the terms behind y_i, i.e. the
+    natural scale of its rounding error (tolerance section)."""
+    a = [np.abs(np.asarray(t, dtype=np.float64)) for t in (x, w3, lam, u)]
+    return fwd(a[0], a[1], a[2], a[3], G, mask,
+               None if h0 is None else np.abs(np.asarray(h0, dtype=np.float64)))
+
+
+def bwd_magnitude(x, w3, lam, u, dy, G: int, mask: int, h0=None):
+    a = [np.abs(np.asarray(t, dtype=np.float64)) for t in (x, w3, lam, u, dy)]
+    return bwd(a[0], a[1], a[2], a[3], a[4], G, mask,
+               None if h0 is None else np.abs(np.asarray(h0, dtype=np.float64)))
