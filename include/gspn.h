@@ -1,0 +1,145 @@
+/*
+ * gspn.h -- C ABI of libgspn: the GSPN 2D line-scan linear propagation
+ * (arxiv/paper_2606_00746, "C-GSPN"), hand-written for NVIDIA B200 (sm_100a).
+ *
+ * The operator (Sec. 3, lines 82-99; Sec. 4.2 Eq. 5;
+ * Eq. 9).  For every direction d in dir_mask, every image b,
+ * every channel c with weight group g = c / (C/G):
+ *
+ *     h_d[s, p] = w3_d[g,0,s,p] * h_d[s-1, p-1]
+ *               + w3_d[g,1,s,p] * h_d[s-1, p  ]
+ *               + w3_d[g,2,s,p] * h_d[s-1, p+1]
+ *               + lambda_d[c,s,p] * x[c,s,p]                  (Eq. 1 / Eq. 5)
+ *     y[c]      = sum_d  u_d[c] (.) h_d[c]                    (Eq. 2, merged as in Eq. 9)
+ *
+ * where s is the scan step and p the position across the scan line:
+ *     T->B : (i,j) = (s, p)            B->T : (i,j) = (H-1-s, p)
+ *     L->R : (i,j) = (p, s)            R->L : (i,j) = (p, W-1-s)
+ * Out-of-grid neighbours contribute 0 and their tap is never read.  h_d[-1] is
+ * h0 (zeros when NULL).  Tap k = 0,1,2 is the neighbour at offset -1,0,+1 along
+ * the NON-scan axis ("top-left, top-center, top-right").
+ * Accumulation is always fp32; the hidden state h is never rounded to the
+ * storage type; every output element is rounded once (RNE) when stored.
+ *
+ * Layouts (all dense, C-contiguous, image layout, D = popcount(dir_mask),
+ * direction slabs in ascending bit order, Lmax = max(H,W)):
+ *     x, y, dy, dx            [B, C, H, W]
+ *     lambda, u, dlambda, du  [D, B, C, H, W]
+ *     w3, dw3                 [D, B, G, 3, H, W]
+ *     h0, dh0                 [D, B, C, Lmax]   (first Lp entries used; dh0's
+ *                                               remaining entries are written 0)
+ *     y_dirs (gspn_merge)     [D, B, C, H, W];  m [D, C] fp32
+ *
+ * Pointers and ownership.  Every pointer of the *device* entry points is a
+ * DEVICE pointer owned by the caller; the library never allocates, frees or
+ * retains device memory in those calls and keeps no state between calls.
+ * `stream` is a cudaStream_t (NULL = the legacy default stream); the calls
+ * enqueue work on it and return without synchronising.  Outputs are fully
+ * overwritten, never accumulated into, and must not alias any input.  Base
+ * pointers must be 16-byte aligned (GSPN_EALIGN otherwise).  The *_host entry
+ * points take HOST pointers with the same layouts; they stage through device
+ * memory obtained from the stream-ordered allocator, copy in, run the device
+ * entry point, copy out, and synchronise the stream before returning.
+ *
+ * Errors.  Every call returns a status code, never throws, never exits.
+ * gspn_last_error() returns a thread-local, NUL-terminated description of the
+ * last non-OK status on the calling thread.
+ *     GSPN_EINVAL        bad shape (B,C,H,W,G < 1, C % G != 0), dir_mask not in
+ *                        [1,15], unknown dtype, NULL required pointer
+ *     GSPN_EUNSUPPORTED  shape outside what the kernels hold on chip (a plane's
+ *                        fp32 accumulator must fit one SM's shared memory;
+ *                        max(H,W) <= 1024)
+ *     GSPN_EALIGN        a base pointer is not 16-byte aligned
+ *     GSPN_ECUDA         a CUDA runtime call or launch failed
+ * There is no CPU fallback: without a CUDA device every compute entry point
+ * returns GSPN_ECUDA.
+ */
+#ifndef GSPN_H_
+#define GSPN_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { GSPN_DIR_TB = 1, GSPN_DIR_BT = 2, GSPN_DIR_LR = 4, GSPN_DIR_RL = 8, GSPN_DIR_ALL = 15 };
+enum { GSPN_F32 = 0, GSPN_BF16 = 1 };   /* storage type of every tensor; arithmetic is fp32 */
+enum { GSPN_OK = 0, GSPN_EINVAL = 1, GSPN_EUNSUPPORTED = 2, GSPN_EALIGN = 3,
+       GSPN_EWORKSPACE = 4, GSPN_ECUDA = 5 };
+/* kernel selection for A/B measurements; GSPN_IMPL_AUTO is what users call */
+enum { GSPN_IMPL_AUTO = 0, GSPN_IMPL_NAIVE = 1, GSPN_IMPL_FUSED = 2 };
+
+/*
+ * Forward scan, Eq. (1),(2),(5),(9): the whole
+ * Ls-step recurrence of every direction in dir_mask and the merge over
+ * directions in ONE launch; x is read once, y written once.
+ */
+int gspn_scan_fwd(const void* x, const void* w3, const void* lambda, const void* u, void* y,
+                  int B, int C, int H, int W, int G, unsigned dir_mask, int dtype, void* stream);
+
+/*
+ * Backward scan: the exact adjoint of gspn_scan_fwd (the paper reports
+ * backward timings only; derivation in DESIGN.md "Backward").
+ * With gy = dy, per direction, in reverse scan order:
+ *     gh[s]      = gy[s]*u[s] + w[s+1]^T gh[s+1]
+ *     du[s]      = gy[s]*h[s]        dlambda[s] = x[s]*gh[s]
+ *     dx[s]     += lambda[s]*gh[s]   (summed over directions)
+ *     dw3[g,k,s,p] = sum_{c in g} gh_c[s,p] * h_c[s-1, p+k-1]
+ *     dh0        = w[0]^T gh[0]
+ * h is recomputed on chip (no saved tensor).  Any output pointer may be NULL
+ * (that output is skipped).
+ */
+int gspn_scan_bwd(const void* x, const void* w3, const void* lambda, const void* u, const void* dy,
+                  void* dx, void* dlambda, void* du, void* dw3, void* dh0,
+                  int B, int C, int H, int W, int G, unsigned dir_mask, int dtype, void* stream);
+
+/*
+ * Merge of per-direction outputs (Eq. 9):
+ *     y[b,c] = sum_q m[q,c] * y_dirs[q,b,c]     (m NULL = ones), fp32 sum, one RNE.
+ */
+int gspn_merge(const void* y_dirs, const float* m, void* y,
+               int B, int C, int H, int W, unsigned dir_mask, int dtype, void* stream);
+
+/* Extended arguments: initial state and kernel selection. */
+typedef struct gspn_args {
+    size_t struct_size;            /* = sizeof(gspn_args_t) */
+    const void *x, *w3, *lambda, *u;
+    const void *h0;                /* [D,B,C,Lmax] or NULL (zeros) */
+    const void *dy;                /* backward only */
+    void *y;                       /* forward only */
+    void *dx, *dlambda, *du, *dw3, *dh0;   /* backward only, each may be NULL */
+    int B, C, H, W, G;
+    unsigned dir_mask;
+    int dtype;
+    int impl;                      /* GSPN_IMPL_* */
+    void *stream;
+} gspn_args_t;
+
+int gspn_scan_fwd_ex(const gspn_args_t* a);
+int gspn_scan_bwd_ex(const gspn_args_t* a);
+
+/* Host-pointer entry points (same layouts, HOST memory; pinned memory makes the copies
+ * asynchronous).  They synchronise `stream` before returning. */
+int gspn_scan_fwd_host(const void* x, const void* w3, const void* lambda, const void* u, void* y,
+                       int B, int C, int H, int W, int G, unsigned dir_mask, int dtype, void* stream);
+int gspn_scan_bwd_host(const void* x, const void* w3, const void* lambda, const void* u, const void* dy,
+                       void* dx, void* dlambda, void* du, void* dw3, void* dh0,
+                       int B, int C, int H, int W, int G, unsigned dir_mask, int dtype, void* stream);
+
+/* Bytes of caller-provided scratch the device entry points need: always 0 in this
+ * version (every intermediate lives on chip); kept so callers can be written once. */
+size_t gspn_workspace_bytes(int B, int C, int H, int W, int G, unsigned dir_mask, int dtype, int is_bwd);
+
+/* Number of kernel launches the last successful call on this thread enqueued. */
+int gspn_last_launch_count(void);
+/* Name of the kernel variant the last successful call on this thread selected. */
+const char* gspn_last_variant(void);
+
+const char* gspn_last_error(void);
+int gspn_version(void);            /* 10000*major + 100*minor + patch */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GSPN_H_ */

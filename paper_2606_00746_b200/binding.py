@@ -1,0 +1,225 @@
+"""Thin Python binding of libgspn (include/gspn.h): argument marshalling only.
+
+Every function here has the name of the C entry point it calls and does no arithmetic of the
+method: tensors are checked (dtype, device, contiguity, shape), their data pointers and the
+current CUDA stream are handed to the C ABI, outputs are allocated with torch (device memory
+only).  There is no fallback: if libgspn.so is missing or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgspn.so")
+
+DIR_TB, DIR_BT, DIR_LR, DIR_RL, DIR_ALL = 1, 2, 4, 8, 15
+F32, BF16 = 0, 1
+IMPL_AUTO, IMPL_NAIVE, IMPL_FUSED = 0, 1, 2
+STATUS = {0: "GSPN_OK", 1: "GSPN_EINVAL", 2: "GSPN_EUNSUPPORTED", 3: "GSPN_EALIGN",
+          4: "GSPN_EWORKSPACE", 5: "GSPN_ECUDA"}
+
+EXPORTS = ("gspn_scan_fwd", "gspn_scan_bwd", "gspn_merge", "gspn_scan_fwd_ex", "gspn_scan_bwd_ex",
+           "gspn_scan_fwd_host", "gspn_scan_bwd_host", "gspn_workspace_bytes",
+           "gspn_last_launch_count", "gspn_last_variant", "gspn_last_error", "gspn_version")
+
+
+class GspnError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class _Args(ctypes.Structure):
+    _fields_ = [("struct_size", ctypes.c_size_t),
+                ("x", ctypes.c_void_p), ("w3", ctypes.c_void_p), ("lam", ctypes.c_void_p),
+                ("u", ctypes.c_void_p), ("h0", ctypes.c_void_p), ("dy", ctypes.c_void_p),
+                ("y", ctypes.c_void_p),
+                ("dx", ctypes.c_void_p), ("dlambda", ctypes.c_void_p), ("du", ctypes.c_void_p),
+                ("dw3", ctypes.c_void_p), ("dh0", ctypes.c_void_p),
+                ("B", ctypes.c_int), ("C", ctypes.c_int), ("H", ctypes.c_int), ("W", ctypes.c_int),
+                ("G", ctypes.c_int), ("dir_mask", ctypes.c_uint), ("dtype", ctypes.c_int),
+                ("impl", ctypes.c_int), ("stream", ctypes.c_void_p)]
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libgspn.so (built in-tree by paper_2606_00746_b200.build); raises if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise GspnError(5, f"{LIB_PATH} not found: run `python -m paper_2606_00746_b200.build` "
+                               "(there is no CPU or PyTorch fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, ci, cu = ctypes.c_void_p, ctypes.c_int, ctypes.c_uint
+        L.gspn_scan_fwd.argtypes = [vp] * 5 + [ci] * 5 + [cu, ci, vp]
+        L.gspn_scan_bwd.argtypes = [vp] * 10 + [ci] * 5 + [cu, ci, vp]
+        L.gspn_merge.argtypes = [vp] * 3 + [ci] * 4 + [cu, ci, vp]
+        L.gspn_scan_fwd_host.argtypes = L.gspn_scan_fwd.argtypes
+        L.gspn_scan_bwd_host.argtypes = L.gspn_scan_bwd.argtypes
+        L.gspn_scan_fwd_ex.argtypes = [ctypes.POINTER(_Args)]
+        L.gspn_scan_bwd_ex.argtypes = [ctypes.POINTER(_Args)]
+        L.gspn_workspace_bytes.argtypes = [ci] * 5 + [cu, ci, ci]
+        L.gspn_workspace_bytes.restype = ctypes.c_size_t
+        L.gspn_last_error.restype = ctypes.c_char_p
+        L.gspn_last_variant.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(rc: int) -> None:
+    if rc != 0:
+        raise GspnError(rc, lib().gspn_last_error().decode())
+
+
+def _dtype_code(t: torch.Tensor) -> int:
+    if t.dtype == torch.float32:
+        return F32
+    if t.dtype == torch.bfloat16:
+        return BF16
+    raise TypeError(f"unsupported storage dtype {t.dtype}")
+
+
+def _popcount(mask: int) -> int:
+    return bin(mask & 15).count("1")
+
+
+def _dev(t, name, shape, like):
+    if t is None:
+        return None
+    if not t.is_cuda or not t.is_contiguous() or t.dtype != like.dtype or t.device != like.device:
+        raise ValueError(f"{name}: need a contiguous CUDA tensor of dtype {like.dtype} on {like.device}")
+    if tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: shape {tuple(t.shape)} != {tuple(shape)}")
+    return t
+
+
+def _p(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(t):
+    return ctypes.c_void_p(torch.cuda.current_stream(t.device).cuda_stream)
+
+
+def _shapes(x, G, dir_mask):
+    B, C, H, W = x.shape
+    D = _popcount(dir_mask)
+    return B, C, H, W, D, (D, B, C, H, W), (D, B, G, 3, H, W), (D, B, C, max(H, W))
+
+
+def gspn_scan_fwd(x, w3, lam, u, G: int, dir_mask: int = DIR_ALL, h0=None, out=None,
+                  impl: int = IMPL_AUTO):
+    """y = sum_d u_d * scan_d(x); see include/gspn.h gspn_scan_fwd / gspn_scan_fwd_ex."""
+    if not x.is_cuda:
+        raise ValueError("x: need a CUDA tensor (there is no CPU path)")
+    B, C, H, W, D, s_bc, s_w, s_h0 = _shapes(x, G, dir_mask)
+    _dev(x, "x", x.shape, x); _dev(w3, "w3", s_w, x); _dev(lam, "lam", s_bc, x); _dev(u, "u", s_bc, x)
+    _dev(h0, "h0", s_h0, x)
+    y = torch.empty_like(x) if out is None else _dev(out, "out", x.shape, x)
+    with torch.cuda.device(x.device):
+        if h0 is None and impl == IMPL_AUTO:
+            rc = lib().gspn_scan_fwd(_p(x), _p(w3), _p(lam), _p(u), _p(y), B, C, H, W, G, dir_mask,
+                                     _dtype_code(x), _stream(x))
+        else:
+            a = _Args(struct_size=ctypes.sizeof(_Args), x=x.data_ptr(), w3=w3.data_ptr(),
+                      lam=lam.data_ptr(), u=u.data_ptr(), h0=None if h0 is None else h0.data_ptr(),
+                      y=y.data_ptr(), B=B, C=C, H=H, W=W, G=G, dir_mask=dir_mask,
+                      dtype=_dtype_code(x), impl=impl,
+                      stream=torch.cuda.current_stream(x.device).cuda_stream)
+            rc = lib().gspn_scan_fwd_ex(ctypes.byref(a))
+    _check(rc)
+    return y
+
+
+def gspn_scan_bwd(x, w3, lam, u, dy, G: int, dir_mask: int = DIR_ALL, h0=None,
+                  need=("dx", "dlambda", "du", "dw3", "dh0"), impl: int = IMPL_AUTO) -> dict:
+    """Adjoint of gspn_scan_fwd; returns the requested gradients (include/gspn.h gspn_scan_bwd)."""
+    if not x.is_cuda:
+        raise ValueError("x: need a CUDA tensor (there is no CPU path)")
+    B, C, H, W, D, s_bc, s_w, s_h0 = _shapes(x, G, dir_mask)
+    _dev(x, "x", x.shape, x); _dev(w3, "w3", s_w, x); _dev(lam, "lam", s_bc, x); _dev(u, "u", s_bc, x)
+    _dev(dy, "dy", x.shape, x); _dev(h0, "h0", s_h0, x)
+    shapes = {"dx": x.shape, "dlambda": s_bc, "du": s_bc, "dw3": s_w, "dh0": s_h0}
+    out = {k: torch.empty(shapes[k], dtype=x.dtype, device=x.device) for k in need}
+    g = lambda k: out[k].data_ptr() if k in out else None
+    with torch.cuda.device(x.device):
+        if h0 is None and impl == IMPL_AUTO:
+            rc = lib().gspn_scan_bwd(_p(x), _p(w3), _p(lam), _p(u), _p(dy), g("dx"), g("dlambda"),
+                                     g("du"), g("dw3"), g("dh0"), B, C, H, W, G, dir_mask,
+                                     _dtype_code(x), _stream(x))
+        else:
+            a = _Args(struct_size=ctypes.sizeof(_Args), x=x.data_ptr(), w3=w3.data_ptr(),
+                      lam=lam.data_ptr(), u=u.data_ptr(), h0=None if h0 is None else h0.data_ptr(),
+                      dy=dy.data_ptr(), dx=g("dx"), dlambda=g("dlambda"), du=g("du"), dw3=g("dw3"),
+                      dh0=g("dh0"), B=B, C=C, H=H, W=W, G=G, dir_mask=dir_mask,
+                      dtype=_dtype_code(x), impl=impl,
+                      stream=torch.cuda.current_stream(x.device).cuda_stream)
+            rc = lib().gspn_scan_bwd_ex(ctypes.byref(a))
+    _check(rc)
+    return out
+
+
+def gspn_merge(y_dirs, m=None, dir_mask: int = DIR_ALL, out=None):
+    """y = sum_q m[q,c] * y_dirs[q]  (include/gspn.h gspn_merge)."""
+    D, B, C, H, W = y_dirs.shape
+    if D != _popcount(dir_mask):
+        raise ValueError("y_dirs: leading dim != popcount(dir_mask)")
+    if not y_dirs.is_cuda or not y_dirs.is_contiguous():
+        raise ValueError("y_dirs: need a contiguous CUDA tensor")
+    if m is not None and (m.dtype != torch.float32 or tuple(m.shape) != (D, C) or not m.is_cuda
+                          or not m.is_contiguous()):
+        raise ValueError("m: need a contiguous CUDA fp32 tensor [D,C]")
+    y = torch.empty((B, C, H, W), dtype=y_dirs.dtype, device=y_dirs.device) if out is None else out
+    with torch.cuda.device(y_dirs.device):
+        rc = lib().gspn_merge(_p(y_dirs), _p(m), _p(y), B, C, H, W, dir_mask, _dtype_code(y_dirs),
+                              _stream(y_dirs))
+    _check(rc)
+    return y
+
+
+def _host(t, name):
+    if t is None:
+        return None
+    if t.is_cuda or not t.is_contiguous():
+        raise ValueError(f"{name}: need a contiguous HOST tensor")
+    return t
+
+
+def gspn_scan_fwd_host(x, w3, lam, u, y, G: int, dir_mask: int = DIR_ALL, stream=None) -> None:
+    """Host-buffer forward (include/gspn.h gspn_scan_fwd_host): H2D, scan, D2H, synchronised."""
+    B, C, H, W = x.shape
+    for t, n in ((x, "x"), (w3, "w3"), (lam, "lam"), (u, "u"), (y, "y")):
+        _host(t, n)
+    st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+    _check(lib().gspn_scan_fwd_host(_p(x), _p(w3), _p(lam), _p(u), _p(y), B, C, H, W, G, dir_mask,
+                                    _dtype_code(x), ctypes.c_void_p(st)))
+
+
+def gspn_scan_bwd_host(x, w3, lam, u, dy, dx, dlambda, du, dw3, dh0, G: int,
+                       dir_mask: int = DIR_ALL, stream=None) -> None:
+    """Host-buffer backward (include/gspn.h gspn_scan_bwd_host)."""
+    B, C, H, W = x.shape
+    for t, n in ((x, "x"), (w3, "w3"), (lam, "lam"), (u, "u"), (dy, "dy"), (dx, "dx"),
+                 (dlambda, "dlambda"), (du, "du"), (dw3, "dw3"), (dh0, "dh0")):
+        _host(t, n)
+    st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+    _check(lib().gspn_scan_bwd_host(_p(x), _p(w3), _p(lam), _p(u), _p(dy), _p(dx), _p(dlambda), _p(du),
+                                    _p(dw3), _p(dh0), B, C, H, W, G, dir_mask, _dtype_code(x),
+                                    ctypes.c_void_p(st)))
+
+
+def gspn_last_launch_count() -> int:
+    return int(lib().gspn_last_launch_count())
+
+
+def gspn_last_variant() -> str:
+    return lib().gspn_last_variant().decode()
+
+
+def gspn_version() -> int:
+    return int(lib().gspn_version())

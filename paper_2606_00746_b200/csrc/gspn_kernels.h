@@ -1,0 +1,26 @@
+// gspn_kernels.h -- host-side launchers of the libgspn kernels (internal to csrc/).
+// Each launcher validates only what its kernel needs (shape already checked by the C ABI),
+// enqueues on `st`, fills LaunchInfo and returns a GSPN_* status.
+#pragma once
+
+#include "gspn_common.cuh"
+
+namespace gspn {
+
+// naive kernels (gspn_naive.cu): one CTA per plane, one thread per cross position, operands read
+// straight from global memory.  Reference GPU path for A/B runs; slow by design.
+template <typename ST> int naive_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
+template <typename ST> int naive_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
+
+// fused kernels (gspn_fused_fwd.cu / gspn_fused_bwd.cu): the hot path.
+template <typename ST> int fused_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
+template <typename ST> int fused_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
+
+// merge (gspn_merge.cu)
+template <typename ST>
+int merge_launch(const ST* y_dirs, const float* m, ST* y, int D, int B, int C, int H, int W,
+                 cudaStream_t st, LaunchInfo* li);
+
+void set_error(const char* fmt, ...);
+
+}  // namespace gspn

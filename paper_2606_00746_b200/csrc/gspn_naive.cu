@@ -1,0 +1,264 @@
+// gspn_naive.cu -- the naive GPU path of libgspn: one CTA per (b,c) plane (forward, backward
+// main) or per (direction, b, group) (weight gradients), one thread per cross position p,
+// operands read straight from global memory, one __syncthreads per scan step.  It exists as the
+// simple-by-construction GPU implementation of Eq. (1),(2),(5) that the
+// fused kernels are A/B-checked against and that serves shapes the fused kernels do not take.
+// Operation order matches a left-to-right evaluation of the recurrence with fused multiply-adds.
+#include "gspn_kernels.h"
+#include "../../include/gspn.h"
+
+namespace gspn {
+
+// one directional forward pass of one plane; every thread of the CTA must call it.
+//   hbuf : 2*(Lmax+2) floats, line s-1 / line s with a zero halo at both ends
+//   hall : NULL or [H*W] floats, receives every hidden state in image layout
+//   ysm  : NULL or [H*W] floats, y += u*h
+template <typename ST>
+__device__ void naive_pass_fwd(int dir, const ST* xp, const ST* wp, const ST* lp, const ST* up,
+                               const ST* h0p, float* hbuf, float* hall, float* ysm, int H, int W) {
+    const int Ls = dir < 2 ? H : W, Lp = dir < 2 ? W : H;
+    const int Lmax = H > W ? H : W;
+    const int plane = H * W;
+    const int p = threadIdx.x;
+    float* cur = hbuf;
+    float* nxt = hbuf + (Lmax + 2);
+    for (int t = p; t < Lmax + 2; t += blockDim.x) { cur[t] = 0.f; nxt[t] = 0.f; }
+    __syncthreads();
+    if (p < Lp && h0p) cur[p + 1] = ld_f(h0p + p);
+    __syncthreads();
+    for (int s = 0; s < Ls; ++s) {
+        if (p < Lp) {
+            const int o = img_off(dir, s, p, H, W);
+            float acc = ld_f(lp + o) * ld_f(xp + o);
+            if (p > 0)      acc = fmaf(ld_f(wp + o), cur[p], acc);
+            acc = fmaf(ld_f(wp + plane + o), cur[p + 1], acc);
+            if (p < Lp - 1) acc = fmaf(ld_f(wp + 2 * plane + o), cur[p + 2], acc);
+            nxt[p + 1] = acc;
+            if (hall) hall[o] = acc;
+            if (ysm) ysm[o] = fmaf(ld_f(up + o), acc, ysm[o]);
+        }
+        __syncthreads();
+        float* t = cur; cur = nxt; nxt = t;
+    }
+}
+
+template <typename ST>
+__global__ void naive_fwd_kernel(FwdArgs<ST> a) {
+    extern __shared__ float smem[];
+    const Shape sh = a.sh;
+    const int H = sh.H, W = sh.W, plane = H * W, Lmax = sh.Lmax();
+    float* ysm = smem;
+    float* hbuf = smem + plane;
+    const int bc = blockIdx.x, b = bc / sh.C, c = bc % sh.C, g = c / sh.cg();
+    for (int o = threadIdx.x; o < plane; o += blockDim.x) ysm[o] = 0.f;
+    __syncthreads();
+    int q = 0;
+    for (int dir = 0; dir < 4; ++dir) {
+        if (!(sh.mask >> dir & 1)) continue;
+        const size_t dbc = ((size_t)q * sh.B + b) * sh.C + c;
+        const size_t dbg = ((size_t)q * sh.B + b) * sh.G + g;
+        naive_pass_fwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + dbg * 3 * plane,
+                           a.lam + dbc * plane, a.u + dbc * plane,
+                           a.h0 ? a.h0 + dbc * Lmax : nullptr, hbuf, nullptr, ysm, H, W);
+        ++q;
+    }
+    __syncthreads();
+    ST* yp = a.y + (size_t)bc * plane;
+    for (int o = threadIdx.x; o < plane; o += blockDim.x) st_f(yp + o, ysm[o]);
+}
+
+// reverse pass of one direction of one plane.  hall holds the forward states of this direction.
+//   dxs  : NULL or [H*W] floats, dx += lambda*gh
+//   dws  : NULL or [3*H*W] floats, dw_k += gh * h[s-1, p+k-1]
+//   ghs  : Lmax+2 floats scratch
+template <typename ST>
+__device__ void naive_pass_bwd(int dir, const ST* xp, const ST* wp, const ST* lp, const ST* up,
+                               const ST* h0p, const ST* gyp, const float* hall, float* ghs,
+                               float* dxs, float* dws, ST* dlp, ST* dup, ST* dh0p, int H, int W) {
+    const int Ls = dir < 2 ? H : W, Lp = dir < 2 ? W : H;
+    const int Lmax = H > W ? H : W;
+    const int plane = H * W;
+    const int p = threadIdx.x;
+    for (int t = p; t < Lmax + 2; t += blockDim.x) ghs[t] = 0.f;
+    float carry = 0.f;
+    __syncthreads();
+    for (int s = Ls - 1; s >= 0; --s) {
+        if (p < Lp) {
+            const int o = img_off(dir, s, p, H, W);
+            const float gy = ld_f(gyp + o);
+            const float gh = fmaf(gy, ld_f(up + o), carry);
+            if (dup) st_f(dup + o, gy * hall[o]);
+            if (dxs) dxs[o] = fmaf(ld_f(lp + o), gh, dxs[o]);
+            if (dlp) st_f(dlp + o, ld_f(xp + o) * gh);
+            if (dws) {
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const int pn = p + k - 1;
+                    if (pn < 0 || pn >= Lp) continue;
+                    float hp;
+                    if (s > 0) hp = hall[img_off(dir, s - 1, pn, H, W)];
+                    else       hp = h0p ? ld_f(h0p + pn) : 0.f;
+                    dws[k * plane + o] = fmaf(gh, hp, dws[k * plane + o]);
+                }
+            }
+            ghs[p + 1] = gh;
+        }
+        __syncthreads();
+        if (p < Lp) {
+            // carry = w[s]^T gh : position p receives from p-1 (its tap k=2), p (k=1), p+1 (k=0)
+            float acc = 0.f;
+            if (p > 0)      acc = fmaf(ld_f(wp + 2 * plane + img_off(dir, s, p - 1, H, W)), ghs[p], acc);
+            acc = fmaf(ld_f(wp + plane + img_off(dir, s, p, H, W)), ghs[p + 1], acc);
+            if (p < Lp - 1) acc = fmaf(ld_f(wp + img_off(dir, s, p + 1, H, W)), ghs[p + 2], acc);
+            carry = acc;
+        }
+        __syncthreads();
+    }
+    if (dh0p) {
+        if (p < Lp) st_f(dh0p + p, carry);
+        else if (p < Lmax) st_f(dh0p + p, 0.f);
+    }
+}
+
+// grid B*C: dx (summed over directions on chip), dlambda, du, dh0
+template <typename ST>
+__global__ void naive_bwd_main_kernel(BwdArgs<ST> a) {
+    extern __shared__ float smem[];
+    const Shape sh = a.sh;
+    const int H = sh.H, W = sh.W, plane = H * W, Lmax = sh.Lmax();
+    float* hall = smem;
+    float* dxs = smem + plane;
+    float* hbuf = dxs + plane;
+    float* ghs = hbuf + 2 * (Lmax + 2);
+    const int bc = blockIdx.x, b = bc / sh.C, c = bc % sh.C, g = c / sh.cg();
+    for (int o = threadIdx.x; o < plane; o += blockDim.x) dxs[o] = 0.f;
+    __syncthreads();
+    int q = 0;
+    for (int dir = 0; dir < 4; ++dir) {
+        if (!(sh.mask >> dir & 1)) continue;
+        const size_t dbc = ((size_t)q * sh.B + b) * sh.C + c;
+        const size_t dbg = ((size_t)q * sh.B + b) * sh.G + g;
+        const ST* h0p = a.h0 ? a.h0 + dbc * Lmax : nullptr;
+        naive_pass_fwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + dbg * 3 * plane,
+                           a.lam + dbc * plane, a.u + dbc * plane, h0p, hbuf, hall, nullptr, H, W);
+        naive_pass_bwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + dbg * 3 * plane,
+                           a.lam + dbc * plane, a.u + dbc * plane, h0p, a.dy + (size_t)bc * plane,
+                           hall, ghs, a.dx ? dxs : nullptr, nullptr,
+                           a.dlam ? a.dlam + dbc * plane : nullptr,
+                           a.du ? a.du + dbc * plane : nullptr,
+                           a.dh0 ? a.dh0 + dbc * Lmax : nullptr, H, W);
+        __syncthreads();
+        ++q;
+    }
+    if (a.dx) {
+        ST* dxp = a.dx + (size_t)bc * plane;
+        for (int o = threadIdx.x; o < plane; o += blockDim.x) st_f(dxp + o, dxs[o]);
+    }
+}
+
+// grid D*B*G: dw3 of one (direction slab, b, group), channels accumulated in ascending order
+template <typename ST>
+__global__ void naive_bwd_dw_kernel(BwdArgs<ST> a) {
+    extern __shared__ float smem[];
+    const Shape sh = a.sh;
+    const int H = sh.H, W = sh.W, plane = H * W, Lmax = sh.Lmax(), cg = sh.cg();
+    float* hall = smem;
+    float* dws = smem + plane;
+    float* hbuf = dws + 3 * plane;
+    float* ghs = hbuf + 2 * (Lmax + 2);
+    const int q = blockIdx.x / (sh.B * sh.G);
+    const int bg = blockIdx.x % (sh.B * sh.G), b = bg / sh.G, g = bg % sh.G;
+    int dir = 0;
+    for (int d = 0, qq = 0; d < 4; ++d)
+        if (sh.mask >> d & 1) { if (qq == q) dir = d; ++qq; }
+    for (int o = threadIdx.x; o < 3 * plane; o += blockDim.x) dws[o] = 0.f;
+    __syncthreads();
+    const size_t dbg = ((size_t)q * sh.B + b) * sh.G + g;
+    for (int cc = 0; cc < cg; ++cc) {
+        const int c = g * cg + cc;
+        const size_t bc = (size_t)b * sh.C + c;
+        const size_t dbc = ((size_t)q * sh.B + b) * sh.C + c;
+        const ST* h0p = a.h0 ? a.h0 + dbc * Lmax : nullptr;
+        naive_pass_fwd<ST>(dir, a.x + bc * plane, a.w3 + dbg * 3 * plane, a.lam + dbc * plane,
+                           a.u + dbc * plane, h0p, hbuf, hall, nullptr, H, W);
+        naive_pass_bwd<ST>(dir, a.x + bc * plane, a.w3 + dbg * 3 * plane, a.lam + dbc * plane,
+                           a.u + dbc * plane, h0p, a.dy + bc * plane, hall, ghs, nullptr, dws,
+                           nullptr, nullptr, nullptr, H, W);
+        __syncthreads();
+    }
+    ST* dwp = a.dw3 + dbg * 3 * plane;
+    for (int o = threadIdx.x; o < 3 * plane; o += blockDim.x) st_f(dwp + o, dws[o]);
+}
+
+static int round_up32(int v) { return (v + 31) / 32 * 32; }
+
+template <typename K>
+static int prep_smem(K kernel, size_t bytes, const char* what) {
+    if (bytes > (size_t)kMaxSmemOptin) {
+        set_error("%s: needs %zu B of shared memory per CTA (> %d)", what, bytes, kMaxSmemOptin);
+        return GSPN_EUNSUPPORTED;
+    }
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e != cudaSuccess) {
+        set_error("%s: cudaFuncSetAttribute: %s", what, cudaGetErrorString(e));
+        return GSPN_ECUDA;
+    }
+    return GSPN_OK;
+}
+
+static int check_launch(const char* what) {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        set_error("%s: launch failed: %s", what, cudaGetErrorString(e));
+        return GSPN_ECUDA;
+    }
+    return GSPN_OK;
+}
+
+template <typename ST>
+int naive_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li) {
+    const Shape& sh = a.sh;
+    if (sh.Lmax() > 1024) { set_error("naive fwd: max(H,W) = %d > 1024", sh.Lmax()); return GSPN_EUNSUPPORTED; }
+    const size_t smem = (sh.plane() + 2 * (sh.Lmax() + 2)) * sizeof(float);
+    int rc = prep_smem(naive_fwd_kernel<ST>, smem, "naive fwd");
+    if (rc) return rc;
+    naive_fwd_kernel<ST><<<sh.B * sh.C, round_up32(sh.Lmax()), smem, st>>>(a);
+    li->launches = 1;
+    li->variant = "naive_fwd";
+    return check_launch("naive fwd");
+}
+
+template <typename ST>
+int naive_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li) {
+    const Shape& sh = a.sh;
+    if (sh.Lmax() > 1024) { set_error("naive bwd: max(H,W) = %d > 1024", sh.Lmax()); return GSPN_EUNSUPPORTED; }
+    const size_t aux = 3 * (sh.Lmax() + 2) * sizeof(float);
+    li->launches = 0;
+    li->variant = "naive_bwd";
+    if (a.dx || a.dlam || a.du || a.dh0) {
+        const size_t smem = 2 * sh.plane() * sizeof(float) + aux;
+        int rc = prep_smem(naive_bwd_main_kernel<ST>, smem, "naive bwd (dx,dlambda,du,dh0)");
+        if (rc) return rc;
+        naive_bwd_main_kernel<ST><<<sh.B * sh.C, round_up32(sh.Lmax()), smem, st>>>(a);
+        ++li->launches;
+        rc = check_launch("naive bwd main");
+        if (rc) return rc;
+    }
+    if (a.dw3) {
+        const size_t smem = 4 * sh.plane() * sizeof(float) + aux;
+        int rc = prep_smem(naive_bwd_dw_kernel<ST>, smem, "naive bwd (dw3)");
+        if (rc) return rc;
+        naive_bwd_dw_kernel<ST><<<sh.D() * sh.B * sh.G, round_up32(sh.Lmax()), smem, st>>>(a);
+        ++li->launches;
+        rc = check_launch("naive bwd dw");
+        if (rc) return rc;
+    }
+    return GSPN_OK;
+}
+
+template int naive_fwd_launch<float>(const FwdArgs<float>&, cudaStream_t, LaunchInfo*);
+template int naive_fwd_launch<__nv_bfloat16>(const FwdArgs<__nv_bfloat16>&, cudaStream_t, LaunchInfo*);
+template int naive_bwd_launch<float>(const BwdArgs<float>&, cudaStream_t, LaunchInfo*);
+template int naive_bwd_launch<__nv_bfloat16>(const BwdArgs<__nv_bfloat16>&, cudaStream_t, LaunchInfo*);
+
+}  // namespace gspn

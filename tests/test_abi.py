@@ -1,0 +1,81 @@
+"""CPU-side checks of the C-ABI boundary: the library builds, loads, exports every symbol that
+include/gspn.h declares, and rejects bad arguments before touching a GPU (no compute calls)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_2606_00746_b200 as gspn
+from paper_2606_00746_b200 import build as gbuild
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    gbuild.build()
+    return gspn.lib()
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "gspn.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(gspn_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_header_symbols_are_exported(L):
+    names = declared_symbols()
+    assert {"gspn_scan_fwd", "gspn_scan_bwd", "gspn_merge"} <= set(names)
+    for n in names:
+        assert hasattr(L, n), f"{n} declared in include/gspn.h but not exported by libgspn.so"
+    assert set(names) == set(gspn.EXPORTS)
+
+
+def test_version_and_workspace(L):
+    assert gspn.gspn_version() >= 100
+    assert L.gspn_workspace_bytes(4, 256, 128, 128, 64, 15, 1, 0) == 0
+    assert L.gspn_workspace_bytes(32, 128, 73, 73, 32, 15, 1, 1) == 0
+
+
+def test_argument_validation_without_gpu(L):
+    buf = ctypes.create_string_buffer(4096 + 16)
+    base = (ctypes.addressof(buf) + 15) & ~15
+    p = ctypes.c_void_p(base)
+    odd = ctypes.c_void_p(base + 2)
+
+    def fwd(B=1, C=4, H=4, W=4, G=2, mask=15, dtype=0, x=p, y=p):
+        return L.gspn_scan_fwd(x, p, p, p, y, B, C, H, W, G, mask, dtype, None)
+
+    assert fwd(B=0) == 1 and b"shape" in L.gspn_last_error()
+    assert fwd(C=4, G=3) == 1 and b"multiple" in L.gspn_last_error()
+    assert fwd(mask=0) == 1 and fwd(mask=16) == 1
+    assert fwd(dtype=7) == 1
+    assert fwd(x=None) == 1 and b"NULL" in L.gspn_last_error()
+    assert fwd(x=odd) == 3 and b"aligned" in L.gspn_last_error()
+    assert L.gspn_scan_bwd(p, p, p, p, None, p, p, p, p, p, 1, 4, 4, 4, 2, 15, 0, None) == 1
+    assert L.gspn_merge(None, None, p, 1, 4, 4, 4, 15, 0, None) == 1
+    # a backward call that asks for no output is a no-op
+    assert L.gspn_scan_bwd(p, p, p, p, p, None, None, None, None, None, 1, 4, 4, 4, 2, 15, 0, None) == 0
+    assert L.gspn_last_launch_count() == 0
+
+
+def test_binding_refuses_cpu_tensors():
+    import torch
+    x = torch.zeros(1, 2, 3, 3)
+    with pytest.raises(ValueError):
+        gspn.gspn_scan_fwd(x, x, x, x, 1)
+
+
+def test_sources_do_not_reference_the_oracle():
+    """The product path and the oracle share no code and neither imports the other."""
+    pkg = os.path.join(ROOT, "paper_2606_00746_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                s = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in s.lower() or f == "README.md", f"{f} mentions the oracle"
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c", ".h")):
+            s = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2606_00746_b200" not in s and "libgspn.so" not in s

@@ -1,0 +1,184 @@
+"""GPU parity: libgspn (through the C ABI) against the fp64 CPU oracle on the same seeded inputs.
+
+Small cases are compared element by element over whole tensors; BASELINE.json's full-size configs
+are launched exactly as bench.py launches them and compared on sampled images (every (b,group)
+unit is independent, so the oracle recomputes whole images).  Gates are in tests/parity_util.py.
+"""
+import numpy as np
+import pytest
+import torch
+
+import gspn_inputs as gi
+import paper_2606_00746_b200 as gspn
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+
+IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO]
+IMPL_IDS = ["naive", "auto"]
+
+# (B, C, H, W, G): degenerate lines, W in {1,2,3}, H != W, beyond one warp, ragged tails, cg in {1,C}
+SMALL_SHAPES = [
+    (1, 1, 1, 1, 1), (1, 2, 1, 5, 1), (1, 2, 5, 1, 2), (2, 4, 4, 2, 2), (1, 3, 3, 3, 1),
+    (2, 4, 5, 7, 2), (2, 4, 7, 5, 4), (1, 8, 16, 16, 8), (1, 4, 33, 35, 1), (2, 6, 40, 24, 3),
+    (1, 4, 27, 27, 1), (1, 2, 73, 73, 2), (1, 8, 56, 56, 1), (1, 2, 128, 128, 1), (1, 2, 64, 130, 2),
+    (1, 2, 100, 36, 1),
+]
+
+
+def _ids(shapes):
+    return ["x".join(map(str, s)) for s in shapes]
+
+
+@pytest.mark.parametrize("impl", IMPLS, ids=IMPL_IDS)
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("shape", SMALL_SHAPES, ids=_ids(SMALL_SHAPES))
+def test_fwd_small_shapes(shape, dtype, impl):
+    cfg = gi.small_config("s", *shape, seed=11)
+    r = pu.check_fwd(cfg, dtype, impl=impl)
+    assert r["ok"], r
+
+
+@pytest.mark.parametrize("impl", IMPLS, ids=IMPL_IDS)
+@pytest.mark.parametrize("mask", [1, 2, 4, 8, 3, 12, 5, 10, 7, 14])
+def test_fwd_direction_masks(mask, impl):
+    for dtype in ("f32", "bf16"):
+        cfg = gi.small_config("m", 2, 4, 9, 12, 2, dir_mask=mask, seed=5 + mask)
+        r = pu.check_fwd(cfg, dtype, impl=impl)
+        assert r["ok"], (dtype, r)
+
+
+@pytest.mark.parametrize("impl", IMPLS, ids=IMPL_IDS)
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_fwd_with_initial_state(dtype, impl):
+    for shape in [(2, 4, 6, 9, 2), (1, 2, 20, 40, 1)]:
+        cfg = gi.small_config("h0", *shape, seed=21)
+        r = pu.check_fwd(cfg, dtype, impl=impl, with_h0=True)
+        assert r["ok"], r
+
+
+@pytest.mark.parametrize("impl", IMPLS, ids=IMPL_IDS)
+def test_cfg1_tiny_forward(impl):
+    """BASELINE.json config 1: B=1, C=8, H=W=16, G=8, fp32, T->B, seed 0."""
+    cfg = gi.CONFIGS["cfg1_tiny"]
+    r = pu.check_fwd(cfg, "f32", impl=impl)
+    assert r["ok"], r
+    # fp32 on the tiny grid also meets BASELINE.json's literal wording on |y| above the floor
+    assert r["max_err_over_A"] <= 1e-6
+
+
+BWD_SHAPES = [
+    (1, 1, 1, 1, 1), (1, 2, 1, 5, 1), (1, 2, 5, 1, 2), (1, 4, 8, 8, 2), (2, 4, 5, 7, 2),
+    (2, 4, 7, 5, 4), (1, 4, 33, 35, 1), (1, 4, 27, 27, 2), (1, 4, 73, 73, 1), (1, 8, 56, 56, 1),
+    (1, 2, 64, 40, 2),
+]
+
+
+@pytest.mark.parametrize("impl", IMPLS, ids=IMPL_IDS)
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("shape", BWD_SHAPES, ids=_ids(BWD_SHAPES))
+def test_bwd_small_shapes(shape, dtype, impl):
+    cfg = gi.small_config("b", *shape, seed=13, backward=True)
+    r = pu.check_bwd(cfg, dtype, impl=impl)
+    assert r["ok"], r
+
+
+@pytest.mark.parametrize("impl", IMPLS, ids=IMPL_IDS)
+@pytest.mark.parametrize("mask", [1, 2, 4, 8, 6, 9, 13])
+def test_bwd_direction_masks_and_h0(mask, impl):
+    cfg = gi.small_config("bm", 2, 4, 9, 12, 2, dir_mask=mask, seed=40 + mask, backward=True)
+    for dtype in ("f32", "bf16"):
+        r = pu.check_bwd(cfg, dtype, impl=impl, with_h0=True)
+        assert r["ok"], (dtype, r)
+
+
+def test_bwd_optional_outputs():
+    cfg = gi.small_config("opt", 1, 4, 8, 8, 2, seed=3, backward=True)
+    t = {k: v.cuda() for k, v in gi.make_inputs(cfg, "f32").items()}
+    full = gspn.gspn_scan_bwd(t["x"], t["w3"], t["lam"], t["u"], t["dy"], cfg.G, cfg.dir_mask)
+    for need in (("dx",), ("dw3",), ("du", "dh0"), ("dlambda", "dw3")):
+        part = gspn.gspn_scan_bwd(t["x"], t["w3"], t["lam"], t["u"], t["dy"], cfg.G, cfg.dir_mask, need=need)
+        assert set(part) == set(need)
+        for k in need:
+            assert torch.equal(part[k], full[k]), k
+
+
+def test_fd_slice_of_cfg5():
+    """BASELINE.json config 5: gradients against central finite differences of the GPU forward
+    itself on a B=1, C=4, H=W=8 slice (fp32 storage, so the differences resolve)."""
+    cfg = gi.small_config("fd", 1, 4, 8, 8, 1, seed=4, backward=True)
+    t = gi.make_inputs(cfg, "f32")
+    d = {k: v.cuda() for k, v in t.items()}
+    g = gspn.gspn_scan_bwd(d["x"], d["w3"], d["lam"], d["u"], d["dy"], cfg.G, cfg.dir_mask)
+    rng = np.random.default_rng(0)
+    eps = 1e-2      # the scan is linear in each operand taken alone: central differences are exact up to rounding
+    for name, key in (("dx", "x"), ("dlambda", "lam"), ("du", "u"), ("dw3", "w3")):
+        base = d[key]
+        for idx in rng.choice(base.numel(), size=12, replace=False):
+            vals = []
+            for sgn in (+1, -1):
+                pert = base.clone()
+                pert.view(-1)[idx] += sgn * eps
+                args = dict(d)
+                args[key] = pert
+                y = gspn.gspn_scan_fwd(args["x"], args["w3"], args["lam"], args["u"], cfg.G, cfg.dir_mask)
+                vals.append(float((y.double() * d["dy"].double()).sum()))
+            fd = (vals[0] - vals[1]) / (2 * eps)
+            got = float(g[name].view(-1)[idx])
+            assert got == pytest.approx(fd, rel=2e-3, abs=2e-3), (name, idx)
+
+
+def test_merge_parity():
+    rng = torch.Generator().manual_seed(7)
+    for dtype, st in (("f32", torch.float32), ("bf16", torch.bfloat16)):
+        for shape, mask in (((4, 2, 6, 8, 8), 15), ((3, 1, 5, 7, 9), 7), ((2, 2, 3, 27, 27), 6), ((1, 1, 1, 1, 1), 8)):
+            D, B, C, H, W = shape
+            yd = torch.randn(shape, generator=rng).to(st)
+            m = torch.randn((D, C), generator=rng)
+            from oracle import gspn_oracle as orc
+            for mm in (None, m):
+                got = gspn.gspn_merge(yd.cuda(), None if mm is None else mm.cuda(), dir_mask=mask)
+                ref = orc.merge(pu.np64(yd), None if mm is None else pu.np64(mm))
+                A = orc.merge(np.abs(pu.np64(yd)), None if mm is None else np.abs(pu.np64(mm)))
+                r = pu.gate(pu.np64(got), ref, A, dtype)
+                assert r["ok"], (shape, dtype, r)
+
+
+FULL = [("cfg2_cls56", "f32"), ("cfg2_cls56", "bf16"), ("cfg3_enc378", "bf16"), ("cfg4_2k", "bf16"),
+        ("cfg5_1k", "bf16")]
+
+
+@pytest.mark.parametrize("name,dtype", FULL, ids=[f"{n}-{d}" for n, d in FULL])
+def test_fwd_full_size_configs(name, dtype):
+    """BASELINE.json configs 2-5 at full size, launched as bench.py launches them."""
+    cfg = gi.CONFIGS[name]
+    t = gi.make_inputs(cfg, dtype, device="cuda:0", with_dy=False)
+    y = gspn.gspn_scan_fwd(t["x"], t["w3"], t["lam"], t["u"], cfg.G, cfg.dir_mask)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(y.float()).all())
+    r = pu.check_fwd_sampled(cfg, dtype, t, y)
+    assert r["ok"], r
+
+
+def test_bwd_full_size_cfg5():
+    """BASELINE.json config 5 (1K forward + backward, bf16) at full size, sampled images."""
+    cfg = gi.CONFIGS["cfg5_1k"]
+    t = gi.make_inputs(cfg, "bf16", device="cuda:0", with_dy=True)
+    g = gspn.gspn_scan_bwd(t["x"], t["w3"], t["lam"], t["u"], t["dy"], cfg.G, cfg.dir_mask)
+    torch.cuda.synchronize()
+    for k, v in g.items():
+        assert bool(torch.isfinite(v.float()).all()), k
+    r = pu.check_bwd_sampled(cfg, "bf16", t, g)
+    assert r["ok"], r
+
+
+def test_stability_property_at_full_size():
+    """Property that holds at any size: with row-stochastic non-negative taps,
+    lambda = u = 1 and x = 1 every direction's h equals the step count + 1, so
+    y[i,j] = (i+1) + (H-i) + (j+1) + (W-j) = H + W + 2 (up to bf16 tap rounding, so fp32 here)."""
+    B, C, H, W, G = 2, 8, 73, 73, 2
+    cfg = gi.small_config("p", B, C, H, W, G, seed=77)
+    t = gi.make_inputs(cfg, "f32", device="cuda:0")
+    ones = torch.ones_like(t["lam"])
+    y = gspn.gspn_scan_fwd(torch.ones_like(t["x"]), t["w3"], ones, ones, G, 15)
+    assert torch.allclose(y, torch.full_like(y, H + W + 2), rtol=1e-5, atol=0)
