@@ -1,0 +1,441 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the GSPN line-scan hot path on B200 against its HBM roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5_1k] [--dtype bf16]
+                    [--impl gspn|reference] [--no-others] [--no-parity]
+
+One "step" is one pass of the whole hot path over one batch of synthetic input of the workload:
+a forward scan and, for a workload with `backward`, the backward scan
+(rows a6-a7).  The default workload is BASELINE.json config 5 (1K grid, forward + backward, bf16
+storage / fp32 accumulation): the one config that exercises every row; the other configs are
+timed forward-only and reported under "others".  Prints ONE JSON line (contract in the task
+statement): value = algorithmic GB/s of the whole job with operands resident in HBM; e2e = the
+same through the host-pointer C-ABI entry points with the copies inside the timed region;
+roofline = the dominant kernel against the measured HBM peak; cpu_baseline = the CPU oracle timed
+on this box's host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+for _p in (ROOT, os.path.join(ROOT, "tests")):
+    if _p not in sys.path:
+        sys.path.insert(0, _p)
+
+METRIC = "GSPN scan achieved HBM GB/s (% of B200 peak) and scan latency ms, fwd and bwd"
+FALLBACK_PEAK_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def peak_hbm():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_PEAK_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="cfg5_1k")
+    ap.add_argument("--dtype", default=None, help="f32|bf16 (default: the workload's last listed dtype)")
+    ap.add_argument("--impl", default="gspn", choices=["gspn", "reference", "naive"])
+    ap.add_argument("--no-others", action="store_true", help="skip the forward-only timings of the other configs")
+    ap.add_argument("--no-parity", action="store_true", help="skip the sampled oracle check of the timed outputs")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks: sampled DURING the timed region through NVML
+class ClockSampler:
+    REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+               0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz, self.ok = [], set(), None, False
+        self._stop = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            visible = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(visible.split(",")[index]) if visible and visible.split(",")[index].isdigit() else index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception as e:       # pragma: no cover
+            self.err = repr(e)
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in self.REASONS.items():
+                    if r & bit and name != "gpu_idle":
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def __enter__(self):
+        if self.ok:
+            self.t = threading.Thread(target=self._run, daemon=True)
+            self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self.ok:
+            self.t.join()
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "note": "NVML unavailable"}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+# ------------------------------------------------------------------------------------------------
+def dist_setup(n_gpus: int):
+    """One process per GPU under torchrun; returns (rank, world, local_rank)."""
+    import torch
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    return rank, world, local
+
+
+def barrier(world):
+    import torch
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    torch.cuda.synchronize()
+
+
+def max_over_ranks(v: float, world: int, device) -> float:
+    import torch
+    if world == 1:
+        return v
+    import torch.distributed as dist
+    t = torch.tensor([v], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands (pinned-order fp32 build, OpenMP over the
+    independent (b,group) units), timed on this box's host cores on the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+    import gspn_inputs as gi
+    from oracle import gspn_oracle as orc
+    cfg = gi.CONFIGS[args.workload]
+    dtype = args.dtype or cfg.dtypes[-1]
+    s = 4 if dtype == "f32" else 2
+    # bounded sample: calibrate on <=2 images, then take as many images per step as keep the whole
+    # (K+W)-step run within ~120 s; K and W are honoured exactly
+    cal_B = min(cfg.B, 2)
+    tc = gi.make_inputs(cfg, dtype, device="cpu", batch_slice=(0, cal_B), with_dy=cfg.backward)
+    ac = {k: v.float().numpy() for k, v in tc.items()}
+    t0 = time.perf_counter()
+    orc.fwd(ac["x"], ac["w3"], ac["lam"], ac["u"], cfg.G, cfg.dir_mask)
+    if cfg.backward:
+        orc.bwd(ac["x"], ac["w3"], ac["lam"], ac["u"], ac["dy"], cfg.G, cfg.dir_mask)
+    per_image = (time.perf_counter() - t0) / cal_B
+    sample_B = int(max(1, min(cfg.B, 120.0 / max(per_image * (args.steps + args.warmup), 1e-9))))
+    sub = gi.with_batch(cfg, sample_B)
+    t = gi.make_inputs(cfg, dtype, device="cpu", batch_slice=(0, sample_B), with_dy=cfg.backward)
+    a = {k: v.float().numpy() for k, v in t.items()}
+    nbytes = sub.fwd_bytes(s) + (sub.bwd_bytes(s) if cfg.backward else 0)
+
+    def step():
+        orc.fwd(a["x"], a["w3"], a["lam"], a["u"], cfg.G, cfg.dir_mask)
+        if cfg.backward:
+            orc.bwd(a["x"], a["w3"], a["lam"], a["u"], a["dy"], cfg.G, cfg.dir_mask)
+
+    steps, warm = max(1, args.steps), max(0, args.warmup)
+    for _ in range(warm):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        step()
+    dt = (time.perf_counter() - t0) / steps
+    gbs = nbytes / dt / 1e9
+    cores = orc.threads()
+    sample = (f"images [0,{sample_B}) of {cfg.name} (B={cfg.B}) per step, fp32 build of the oracle, "
+              f"fwd{'+bwd' if cfg.backward else ''}")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": gbs, "unit": "GB/s", "n_gpus": args.gpus,
+        "steps": steps, "warmup": warm, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg.name, "B": cfg.B, "C": cfg.C, "H": cfg.H, "W": cfg.W, "G": cfg.G,
+                   "dir_mask": cfg.dir_mask, "storage": dtype, "pass": "fwd+bwd" if cfg.backward else "fwd"},
+        "pxch_per_s": sub.n / dt,
+        "cpu_baseline": {"value": gbs, "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": gbs, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def time_cpu_oracle(cfg, dtype, budget_s=12.0):
+    """cpu_baseline leg: the oracle (fp32 build) on the workload, repeated within a time budget."""
+    import gspn_inputs as gi
+    from oracle import gspn_oracle as orc
+    s = 4 if dtype == "f32" else 2
+    t = gi.make_inputs(cfg, dtype, device="cpu", with_dy=cfg.backward)
+    a = {k: v.float().numpy() for k, v in t.items()}
+    nbytes = cfg.fwd_bytes(s) + (cfg.bwd_bytes(s) if cfg.backward else 0)
+    times = []
+    t_end = time.perf_counter() + budget_s
+    while len(times) < 2 or (time.perf_counter() < t_end and len(times) < 8):
+        t0 = time.perf_counter()
+        orc.fwd(a["x"], a["w3"], a["lam"], a["u"], cfg.G, cfg.dir_mask)
+        if cfg.backward:
+            orc.bwd(a["x"], a["w3"], a["lam"], a["u"], a["dy"], cfg.G, cfg.dir_mask)
+        times.append(time.perf_counter() - t0)
+    dt = min(times[1:]) if len(times) > 1 else times[0]
+    return {"value": nbytes / dt / 1e9, "unit": "GB/s", "cores": orc.threads(), "kind": "oracle",
+            "ms_per_step": dt * 1e3, "pxch_per_s": cfg.n / dt,
+            "sample": f"full workload {cfg.name} (B={cfg.B}), fp32 build, fwd{'+bwd' if cfg.backward else ''}, "
+                      f"best of {len(times) - 1} after 1 warm-up"}
+
+
+# ------------------------------------------------------------------------------------------------
+def time_config(gspn, torch, cfg, dtype, steps, warmup, world, impl, want_bwd, tensors=None):
+    """Times `steps` steps (fwd [+ bwd]) of cfg with CUDA events on the launching stream.
+    Returns (dict of timings, tensors, last outputs)."""
+    dev = torch.device("cuda", torch.cuda.current_device())
+    if tensors is None:
+        tensors = __import__("gspn_inputs").make_inputs(cfg, dtype, device=dev, with_dy=want_bwd)
+    t = tensors
+    y = torch.empty_like(t["x"])
+    grads = None
+    launches = 0
+
+    def step(record=None):
+        nonlocal grads, launches
+        if record:
+            record[0].record()
+        gspn.gspn_scan_fwd(t["x"], t["w3"], t["lam"], t["u"], cfg.G, cfg.dir_mask, out=y, impl=impl)
+        launches += gspn.gspn_last_launch_count()
+        variant_f = gspn.gspn_last_variant()
+        if record:
+            record[1].record()
+        variant_b = None
+        if want_bwd:
+            grads = gspn.gspn_scan_bwd(t["x"], t["w3"], t["lam"], t["u"], t["dy"], cfg.G, cfg.dir_mask, impl=impl)
+            launches += gspn.gspn_last_launch_count()
+            variant_b = gspn.gspn_last_variant()
+        if record:
+            record[2].record()
+        return variant_f, variant_b
+
+    for _ in range(warmup):
+        vf, vb = step()
+    launches = 0
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+    barrier(world)
+    t0 = time.perf_counter()
+    for k in range(steps):
+        vf, vb = step(ev[k])
+    barrier(world)
+    wall = time.perf_counter() - t0
+    total_ms = ev[0][0].elapsed_time(ev[-1][2])
+    fwd_ms = sorted(e[0].elapsed_time(e[1]) for e in ev)
+    bwd_ms = sorted(e[1].elapsed_time(e[2]) for e in ev) if want_bwd else None
+    total_ms = max_over_ranks(total_ms, world, dev)
+    res = {"total_ms": total_ms, "ms_per_step": total_ms / steps, "wall_ms": wall * 1e3,
+           "fwd_ms_mean": sum(fwd_ms) / steps, "fwd_ms_median": fwd_ms[steps // 2], "fwd_ms_min": fwd_ms[0],
+           "launches": launches, "variant_fwd": vf, "variant_bwd": vb}
+    if want_bwd:
+        res.update({"bwd_ms_mean": sum(bwd_ms) / steps, "bwd_ms_median": bwd_ms[steps // 2], "bwd_ms_min": bwd_ms[0]})
+    return res, tensors, y, grads
+
+
+def time_e2e(gspn, torch, cfg, dtype, steps, warmup, world, want_bwd, tensors):
+    """Same metric through the host-pointer C-ABI entry points: pinned host operands, H2D copies,
+    kernels and D2H copies of every output inside the timed region."""
+    host = {k: v.cpu().pin_memory() for k, v in tensors.items()}
+    y = torch.empty_like(host["x"]).pin_memory()
+    outs = None
+    if want_bwd:
+        L = max(cfg.H, cfg.W)
+        shp = {"dx": host["x"].shape, "dlambda": host["lam"].shape, "du": host["u"].shape,
+               "dw3": host["w3"].shape, "dh0": (cfg.D, cfg.B, cfg.C, L)}
+        outs = {k: torch.empty(v, dtype=host["x"].dtype).pin_memory() for k, v in shp.items()}
+    nb = lambda t: t.numel() * t.element_size()
+    h2d = sum(nb(host[k]) for k in ("x", "w3", "lam", "u"))
+    d2h = nb(y)
+    if want_bwd:
+        h2d += sum(nb(host[k]) for k in ("x", "w3", "lam", "u", "dy"))
+        d2h += sum(nb(v) for v in outs.values())
+
+    def step():
+        gspn.gspn_scan_fwd_host(host["x"], host["w3"], host["lam"], host["u"], y, cfg.G, cfg.dir_mask)
+        if want_bwd:
+            gspn.gspn_scan_bwd_host(host["x"], host["w3"], host["lam"], host["u"], host["dy"], outs["dx"],
+                                    outs["dlambda"], outs["du"], outs["dw3"], outs["dh0"], cfg.G, cfg.dir_mask)
+
+    for _ in range(max(1, min(warmup, 3))):
+        step()
+    n = max(3, min(steps, 10))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier(world)
+    e0.record()
+    for _ in range(n):
+        step()
+    e1.record()
+    barrier(world)
+    ms = max_over_ranks(e0.elapsed_time(e1), world, torch.device("cuda", torch.cuda.current_device())) / n
+    return ms, h2d, d2h, y, outs, n
+
+
+# ------------------------------------------------------------------------------------------------
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    import torch
+    import gspn_inputs as gi
+    import paper_2606_00746_b200 as gspn
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU path; use --impl reference for the oracle)")
+    gspn.lib()      # raises if libgspn.so is missing: no fallback
+    rank, world, local = dist_setup(args.gpus)
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    impl = gspn.IMPL_NAIVE if args.impl == "naive" else gspn.IMPL_AUTO
+
+    base = gi.CONFIGS[args.workload]
+    dtype = args.dtype or base.dtypes[-1]
+    s = 4 if dtype == "f32" else 2
+    # weak scaling: every rank owns B images of a conceptual world*B batch ((b,group)
+    # units are independent, no collective on the data path); rank r draws its own seed
+    from dataclasses import replace
+    cfg = replace(base, seed=base.seed + 1000 * rank)
+    want_bwd = cfg.backward
+    peak, peak_src = peak_hbm()
+    steps, warmup = max(1, args.steps), max(3, args.warmup)
+
+    with ClockSampler(local) as clk:
+        res, tensors, y, grads = time_config(gspn, torch, cfg, dtype, steps, warmup, world, impl, want_bwd)
+    clocks = clk.summary()
+
+    fwd_b = cfg.fwd_bytes(s)
+    bwd_b = cfg.bwd_bytes(s) if want_bwd else 0
+    step_bytes = fwd_b + bwd_b
+    value = world * step_bytes / (res["ms_per_step"] * 1e-3) / 1e9
+
+    kernels = {"fwd": {"variant": res["variant_fwd"], "ms_mean": res["fwd_ms_mean"], "ms_median": res["fwd_ms_median"],
+                       "ms_min": res["fwd_ms_min"], "alg_bytes": fwd_b,
+                       "gbs": fwd_b / (res["fwd_ms_mean"] * 1e-3) / 1e9,
+                       "frac": fwd_b / (res["fwd_ms_mean"] * 1e-3) / 1e9 / peak}}
+    if want_bwd:
+        kernels["bwd"] = {"variant": res["variant_bwd"], "ms_mean": res["bwd_ms_mean"], "ms_median": res["bwd_ms_median"],
+                          "ms_min": res["bwd_ms_min"], "alg_bytes": bwd_b,
+                          "gbs": bwd_b / (res["bwd_ms_mean"] * 1e-3) / 1e9,
+                          "frac": bwd_b / (res["bwd_ms_mean"] * 1e-3) / 1e9 / peak}
+    dom = max(kernels, key=lambda k: kernels[k]["ms_mean"])
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")      # written by hand from an `ncu --set full` capture
+    try:
+        with open(tpath) as f:
+            traffic = json.load(f).get(f"{cfg.name}:{dtype}:{kernels[dom]['variant']}")
+    except Exception:
+        pass
+    roofline = {"bound": "hbm", "kernel": kernels[dom]["variant"], "pass": dom,
+                "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s", "frac": kernels[dom]["frac"],
+                "traffic": traffic, "peak_source": peak_src,
+                "alg_bytes_per_launch": kernels[dom]["alg_bytes"], "ms_per_launch": kernels[dom]["ms_mean"]}
+
+    parity = None
+    if not args.no_parity and rank == 0:
+        import parity_util as pu
+        pf = pu.check_fwd_sampled(cfg, dtype, tensors, y)
+        parity = {"fwd_ok": pf["ok"], "fwd_max_err_over_A": max(r["max_err_over_A"] for r in pf["slices"])}
+        if want_bwd:
+            pb = pu.check_bwd_sampled(cfg, dtype, tensors, grads)
+            parity["bwd_ok"] = pb["ok"]
+        parity["sample"] = "images first/middle/last of the timed outputs vs the fp64 oracle (tests/parity_util.py gates)"
+
+    e2e = None
+    if not args.no_e2e:
+        ms, h2d, d2h, _, _, n_e2e = time_e2e(gspn, torch, cfg, dtype, steps, warmup, world, want_bwd, tensors)
+        e2e = {"value": world * step_bytes / (ms * 1e-3) / 1e9, "unit": "GB/s", "ms_per_step": ms,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e,
+               "api": "gspn_scan_fwd_host" + (" + gspn_scan_bwd_host" if want_bwd else "")}
+    del grads, y
+
+    others = None
+    if not args.no_others and world == 1:
+        others = {}
+        del tensors
+        torch.cuda.empty_cache()
+        for name, oc in gi.CONFIGS.items():
+            for dt in oc.dtypes:
+                if name == cfg.name and dt == dtype:
+                    continue
+                so = 4 if dt == "f32" else 2
+                r, tt, yy, gg = time_config(gspn, torch, oc, dt, max(5, min(steps, 20)), 3, 1, impl, False)
+                fb = oc.fwd_bytes(so)
+                others[f"{name}:{dt}:fwd"] = {"variant": r["variant_fwd"], "ms": r["fwd_ms_mean"], "ms_min": r["fwd_ms_min"],
+                                               "gbs": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9,
+                                               "frac": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9 / peak,
+                                               "pxch_per_s": oc.n / (r["fwd_ms_mean"] * 1e-3)}
+                del tt, yy, gg
+                torch.cuda.empty_cache()
+
+    cpu = None
+    if not args.no_cpu and rank == 0 and world == 1:
+        cpu = time_cpu_oracle(base, dtype)
+
+    if rank == 0:
+        out = {
+            "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": steps, "warmup": warmup,
+            "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg.name, "B": cfg.B, "C": cfg.C, "H": cfg.H, "W": cfg.W, "G": cfg.G,
+                       "dir_mask": cfg.dir_mask, "storage": dtype, "pass": "fwd+bwd" if want_bwd else "fwd",
+                       "l2": f"operands {step_bytes / 1e6:.0f} MB per step > 126 MB L2 (no flush needed)",
+                       "per_rank_batch": cfg.B},
+            "frac_of_peak": value / world / peak, "pxch_per_s": world * cfg.n / (res["ms_per_step"] * 1e-3),
+            "kernels": kernels, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": res["launches"], "clocks": clocks, "parity": parity, "others": others,
+            "wall_ms_per_step": res["wall_ms"] / steps,
+        }
+        print(json.dumps(out))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
