@@ -56,8 +56,11 @@ static int fwd_typed(const gspn_args_t* a) {
     int rc;
     if (a->impl == GSPN_IMPL_NAIVE) {
         rc = naive_fwd_launch<ST>(f, st, &li);
+    } else if (a->impl == GSPN_IMPL_FLAT) {
+        rc = flat_fwd_launch<ST>(f, st, &li);
     } else {
         rc = fused_fwd_launch<ST>(f, st, &li);
+        if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = flat_fwd_launch<ST>(f, st, &li);
         if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = naive_fwd_launch<ST>(f, st, &li);
     }
     if (rc == GSPN_OK) { g_launches = li.launches; g_variant = li.variant; }
@@ -75,7 +78,7 @@ static int bwd_typed(const gspn_args_t* a) {
     cudaStream_t st = (cudaStream_t)a->stream;
     LaunchInfo li{0, ""};
     int rc;
-    if (a->impl == GSPN_IMPL_NAIVE) {
+    if (a->impl == GSPN_IMPL_NAIVE || a->impl == GSPN_IMPL_FLAT) {
         rc = naive_bwd_launch<ST>(f, st, &li);
     } else {
         rc = fused_bwd_launch<ST>(f, st, &li);
@@ -91,7 +94,7 @@ static int check_ex(const gspn_args_t* a) {
         set_error("gspn_args_t.struct_size=%zu, expected %zu", a->struct_size, sizeof(gspn_args_t));
         return GSPN_EINVAL;
     }
-    if (a->impl < GSPN_IMPL_AUTO || a->impl > GSPN_IMPL_FUSED) {
+    if (a->impl < GSPN_IMPL_AUTO || a->impl > GSPN_IMPL_FLAT) {
         set_error("unknown impl %d", a->impl);
         return GSPN_EINVAL;
     }

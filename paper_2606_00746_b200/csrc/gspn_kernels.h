@@ -16,6 +16,10 @@ template <typename ST> int naive_bwd_launch(const BwdArgs<ST>& a, cudaStream_t s
 template <typename ST> int fused_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 template <typename ST> int fused_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 
+// flat kernels (gspn_flat_fwd.cu / gspn_flat_bwd.cu): fused single-launch kernels for ANY H, W and
+// storage type (rows / planes need not be 16-byte aligned).
+template <typename ST> int flat_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
+
 // merge (gspn_merge.cu)
 template <typename ST>
 int merge_launch(const ST* y_dirs, const float* m, ST* y, int D, int B, int C, int H, int W,

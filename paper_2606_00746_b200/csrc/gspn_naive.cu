@@ -1,6 +1,7 @@
 // gspn_naive.cu -- the naive GPU path of libgspn: one CTA per (b,c) plane (forward, backward
 // main) or per (direction, b, group) (weight gradients), one thread per cross position p,
-// operands read straight from global memory, one __syncthreads per scan step.  It exists as the
+// operands read straight from global memory (a thread fetches the operands of kChunk consecutive
+// steps together, so the global latency is paid once per chunk), one __syncthreads per scan step.  It exists as the
 // simple-by-construction GPU implementation of Eq. (1),(2),(5) that the
 // fused kernels are A/B-checked against and that serves shapes the fused kernels do not take.
 // Operation order matches a left-to-right evaluation of the recurrence with fused multiply-adds.
@@ -13,6 +14,8 @@ namespace gspn {
 //   hbuf : 2*(Lmax+2) floats, line s-1 / line s with a zero halo at both ends
 //   hall : NULL or [H*W] floats, receives every hidden state in image layout
 //   ysm  : NULL or [H*W] floats, y += u*h
+constexpr int kChunk = 8;      // scan steps whose operands a thread fetches together (one global latency per chunk)
+
 template <typename ST>
 __device__ void naive_pass_fwd(int dir, const ST* xp, const ST* wp, const ST* lp, const ST* up,
                                const ST* h0p, float* hbuf, float* hall, float* ysm, int H, int W) {
@@ -26,19 +29,39 @@ __device__ void naive_pass_fwd(int dir, const ST* xp, const ST* wp, const ST* lp
     __syncthreads();
     if (p < Lp && h0p) cur[p + 1] = ld_f(h0p + p);
     __syncthreads();
-    for (int s = 0; s < Ls; ++s) {
-        if (p < Lp) {
-            const int o = img_off(dir, s, p, H, W);
-            float acc = ld_f(lp + o) * ld_f(xp + o);
-            if (p > 0)      acc = fmaf(ld_f(wp + o), cur[p], acc);
-            acc = fmaf(ld_f(wp + plane + o), cur[p + 1], acc);
-            if (p < Lp - 1) acc = fmaf(ld_f(wp + 2 * plane + o), cur[p + 2], acc);
-            nxt[p + 1] = acc;
-            if (hall) hall[o] = acc;
-            if (ysm) ysm[o] = fmaf(ld_f(up + o), acc, ysm[o]);
+    for (int s0 = 0; s0 < Ls; s0 += kChunk) {
+        // operands of steps s0 .. s0+kChunk-1 of this thread's position: all loads in flight at once
+        float lx[kChunk], w0[kChunk], w1[kChunk], w2[kChunk], uu[kChunk];
+#pragma unroll
+        for (int j = 0; j < kChunk; ++j) {
+            lx[j] = w0[j] = w1[j] = w2[j] = uu[j] = 0.f;
+            if (p < Lp && s0 + j < Ls) {
+                const int o = img_off(dir, s0 + j, p, H, W);
+                lx[j] = ld_f(lp + o) * ld_f(xp + o);
+                if (p > 0) w0[j] = ld_f(wp + o);
+                w1[j] = ld_f(wp + plane + o);
+                if (p < Lp - 1) w2[j] = ld_f(wp + 2 * plane + o);
+                if (ysm) uu[j] = ld_f(up + o);
+            }
         }
-        __syncthreads();
-        float* t = cur; cur = nxt; nxt = t;
+#pragma unroll
+        for (int j = 0; j < kChunk; ++j) {
+            const int s = s0 + j;
+            if (s < Ls) {                                   // uniform over the CTA
+                if (p < Lp) {
+                    const int o = img_off(dir, s, p, H, W);
+                    float acc = lx[j];
+                    if (p > 0)      acc = fmaf(w0[j], cur[p], acc);
+                    acc = fmaf(w1[j], cur[p + 1], acc);
+                    if (p < Lp - 1) acc = fmaf(w2[j], cur[p + 2], acc);
+                    nxt[p + 1] = acc;
+                    if (hall) hall[o] = acc;
+                    if (ysm) ysm[o] = fmaf(uu[j], acc, ysm[o]);
+                }
+                __syncthreads();
+                float* t = cur; cur = nxt; nxt = t;
+            }
+        }
     }
 }
 
@@ -82,37 +105,58 @@ __device__ void naive_pass_bwd(int dir, const ST* xp, const ST* wp, const ST* lp
     for (int t = p; t < Lmax + 2; t += blockDim.x) ghs[t] = 0.f;
     float carry = 0.f;
     __syncthreads();
-    for (int s = Ls - 1; s >= 0; --s) {
-        if (p < Lp) {
-            const int o = img_off(dir, s, p, H, W);
-            const float gy = ld_f(gyp + o);
-            const float gh = fmaf(gy, ld_f(up + o), carry);
-            if (dup) st_f(dup + o, gy * hall[o]);
-            if (dxs) dxs[o] = fmaf(ld_f(lp + o), gh, dxs[o]);
-            if (dlp) st_f(dlp + o, ld_f(xp + o) * gh);
-            if (dws) {
+    for (int s1 = Ls - 1; s1 >= 0; s1 -= kChunk) {
+        // operands of steps s1, s1-1, .. s1-kChunk+1: all loads in flight at once
+        float gyv[kChunk], uv[kChunk], lv[kChunk], xv[kChunk], wl[kChunk], wc[kChunk], wr[kChunk];
 #pragma unroll
-                for (int k = 0; k < 3; ++k) {
-                    const int pn = p + k - 1;
-                    if (pn < 0 || pn >= Lp) continue;
-                    float hp;
-                    if (s > 0) hp = hall[img_off(dir, s - 1, pn, H, W)];
-                    else       hp = h0p ? ld_f(h0p + pn) : 0.f;
-                    dws[k * plane + o] = fmaf(gh, hp, dws[k * plane + o]);
-                }
+        for (int j = 0; j < kChunk; ++j) {
+            gyv[j] = uv[j] = lv[j] = xv[j] = wl[j] = wc[j] = wr[j] = 0.f;
+            const int s = s1 - j;
+            if (p < Lp && s >= 0) {
+                const int o = img_off(dir, s, p, H, W);
+                gyv[j] = ld_f(gyp + o); uv[j] = ld_f(up + o);
+                lv[j] = ld_f(lp + o);   xv[j] = ld_f(xp + o);
+                // taps of the carry w[s]^T gh: position p receives from p-1 (its tap k=2), p (k=1), p+1 (k=0)
+                if (p > 0)      wl[j] = ld_f(wp + 2 * plane + img_off(dir, s, p - 1, H, W));
+                wc[j] = ld_f(wp + plane + o);
+                if (p < Lp - 1) wr[j] = ld_f(wp + img_off(dir, s, p + 1, H, W));
             }
-            ghs[p + 1] = gh;
         }
-        __syncthreads();
-        if (p < Lp) {
-            // carry = w[s]^T gh : position p receives from p-1 (its tap k=2), p (k=1), p+1 (k=0)
-            float acc = 0.f;
-            if (p > 0)      acc = fmaf(ld_f(wp + 2 * plane + img_off(dir, s, p - 1, H, W)), ghs[p], acc);
-            acc = fmaf(ld_f(wp + plane + img_off(dir, s, p, H, W)), ghs[p + 1], acc);
-            if (p < Lp - 1) acc = fmaf(ld_f(wp + img_off(dir, s, p + 1, H, W)), ghs[p + 2], acc);
-            carry = acc;
+#pragma unroll
+        for (int j = 0; j < kChunk; ++j) {
+            const int s = s1 - j;
+            if (s >= 0) {                                   // uniform over the CTA
+                if (p < Lp) {
+                    const int o = img_off(dir, s, p, H, W);
+                    const float gy = gyv[j];
+                    const float gh = fmaf(gy, uv[j], carry);
+                    if (dup) st_f(dup + o, gy * hall[o]);
+                    if (dxs) dxs[o] = fmaf(lv[j], gh, dxs[o]);
+                    if (dlp) st_f(dlp + o, xv[j] * gh);
+                    if (dws) {
+#pragma unroll
+                        for (int k = 0; k < 3; ++k) {
+                            const int pn = p + k - 1;
+                            if (pn < 0 || pn >= Lp) continue;
+                            float hp;
+                            if (s > 0) hp = hall[img_off(dir, s - 1, pn, H, W)];
+                            else       hp = h0p ? ld_f(h0p + pn) : 0.f;
+                            dws[k * plane + o] = fmaf(gh, hp, dws[k * plane + o]);
+                        }
+                    }
+                    ghs[p + 1] = gh;
+                }
+                __syncthreads();
+                if (p < Lp) {
+                    float acc = 0.f;
+                    if (p > 0)      acc = fmaf(wl[j], ghs[p], acc);
+                    acc = fmaf(wc[j], ghs[p + 1], acc);
+                    if (p < Lp - 1) acc = fmaf(wr[j], ghs[p + 2], acc);
+                    carry = acc;
+                }
+                __syncthreads();
+            }
         }
-        __syncthreads();
     }
     if (dh0p) {
         if (p < Lp) st_f(dh0p + p, carry);

@@ -16,6 +16,8 @@ pytestmark = pytest.mark.gpu
 
 IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO]
 IMPL_IDS = ["naive", "auto"]
+FWD_IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO, gspn.IMPL_FLAT]
+FWD_IMPL_IDS = ["naive", "auto", "flat"]
 
 # (B, C, H, W, G): degenerate lines, W in {1,2,3}, H != W, beyond one warp, ragged tails, cg in {1,C}
 SMALL_SHAPES = [
@@ -30,7 +32,7 @@ def _ids(shapes):
     return ["x".join(map(str, s)) for s in shapes]
 
 
-@pytest.mark.parametrize("impl", IMPLS, ids=IMPL_IDS)
+@pytest.mark.parametrize("impl", FWD_IMPLS, ids=FWD_IMPL_IDS)
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
 @pytest.mark.parametrize("shape", SMALL_SHAPES, ids=_ids(SMALL_SHAPES))
 def test_fwd_small_shapes(shape, dtype, impl):
@@ -39,7 +41,7 @@ def test_fwd_small_shapes(shape, dtype, impl):
     assert r["ok"], r
 
 
-@pytest.mark.parametrize("impl", IMPLS, ids=IMPL_IDS)
+@pytest.mark.parametrize("impl", FWD_IMPLS, ids=FWD_IMPL_IDS)
 @pytest.mark.parametrize("mask", [1, 2, 4, 8, 3, 12, 5, 10, 7, 14])
 def test_fwd_direction_masks(mask, impl):
     for dtype in ("f32", "bf16"):
@@ -48,7 +50,7 @@ def test_fwd_direction_masks(mask, impl):
         assert r["ok"], (dtype, r)
 
 
-@pytest.mark.parametrize("impl", IMPLS, ids=IMPL_IDS)
+@pytest.mark.parametrize("impl", FWD_IMPLS, ids=FWD_IMPL_IDS)
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
 def test_fwd_with_initial_state(dtype, impl):
     for shape in [(2, 4, 6, 9, 2), (1, 2, 20, 40, 1)]:
@@ -57,7 +59,7 @@ def test_fwd_with_initial_state(dtype, impl):
         assert r["ok"], r
 
 
-@pytest.mark.parametrize("impl", IMPLS, ids=IMPL_IDS)
+@pytest.mark.parametrize("impl", FWD_IMPLS, ids=FWD_IMPL_IDS)
 def test_cfg1_tiny_forward(impl):
     """BASELINE.json config 1: B=1, C=8, H=W=16, G=8, fp32, T->B, seed 0."""
     cfg = gi.CONFIGS["cfg1_tiny"]
