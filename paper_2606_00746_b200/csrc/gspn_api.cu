@@ -78,7 +78,7 @@ static int bwd_typed(const gspn_args_t* a) {
     cudaStream_t st = (cudaStream_t)a->stream;
     LaunchInfo li{0, ""};
     int rc;
-    if (a->impl == GSPN_IMPL_NAIVE || a->impl == GSPN_IMPL_FLAT) {
+    if (a->impl == GSPN_IMPL_NAIVE) {
         rc = naive_bwd_launch<ST>(f, st, &li);
     } else {
         rc = fused_bwd_launch<ST>(f, st, &li);

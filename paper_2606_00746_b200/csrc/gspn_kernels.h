@@ -12,7 +12,7 @@ namespace gspn {
 template <typename ST> int naive_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 template <typename ST> int naive_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 
-// fused kernels (gspn_fused_fwd.cu / gspn_fused_bwd.cu): the hot path.
+// fused kernels: forward tile kernel (gspn_fused_fwd.cu), backward group kernel (gspn_group_bwd.cu).
 template <typename ST> int fused_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 template <typename ST> int fused_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 

@@ -184,3 +184,15 @@ def test_stability_property_at_full_size():
     ones = torch.ones_like(t["lam"])
     y = gspn.gspn_scan_fwd(torch.ones_like(t["x"]), t["w3"], ones, ones, G, 15)
     assert torch.allclose(y, torch.full_like(y, H + W + 2), rtol=1e-5, atol=0)
+
+
+def test_auto_selects_fused_kernels_where_supported():
+    """GSPN_IMPL_AUTO must run the fused single-launch kernels on the benchmark shapes (no silent
+    fallback to the naive path): 73x73 with 4 channels per group, forward and backward."""
+    cfg = gi.small_config("sel", 1, 8, 73, 73, 2, seed=9, backward=True)
+    r = pu.check_bwd(cfg, "bf16")
+    assert r["ok"], r
+    assert r["variant"] == "fused_bwd_group", r["variant"]
+    assert gspn.gspn_last_launch_count() == 1
+    r = pu.check_fwd(cfg, "bf16")
+    assert r["ok"] and r["variant"] == "fused_fwd_flat", r
