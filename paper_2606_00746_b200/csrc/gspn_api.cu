@@ -80,8 +80,11 @@ static int bwd_typed(const gspn_args_t* a) {
     int rc;
     if (a->impl == GSPN_IMPL_NAIVE) {
         rc = naive_bwd_launch<ST>(f, st, &li);
-    } else {
+    } else if (a->impl == GSPN_IMPL_FUSED) {
         rc = fused_bwd_launch<ST>(f, st, &li);
+    } else {
+        rc = chain_bwd_launch<ST>(f, st, &li);
+        if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = fused_bwd_launch<ST>(f, st, &li);
         if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = naive_bwd_launch<ST>(f, st, &li);
     }
     if (rc == GSPN_OK) { g_launches = li.launches; g_variant = li.variant; }
@@ -94,7 +97,7 @@ static int check_ex(const gspn_args_t* a) {
         set_error("gspn_args_t.struct_size=%zu, expected %zu", a->struct_size, sizeof(gspn_args_t));
         return GSPN_EINVAL;
     }
-    if (a->impl < GSPN_IMPL_AUTO || a->impl > GSPN_IMPL_FLAT) {
+    if (a->impl < GSPN_IMPL_AUTO || a->impl > GSPN_IMPL_CHAIN) {
         set_error("unknown impl %d", a->impl);
         return GSPN_EINVAL;
     }

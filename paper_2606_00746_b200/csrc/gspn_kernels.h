@@ -20,6 +20,10 @@ template <typename ST> int fused_bwd_launch(const BwdArgs<ST>& a, cudaStream_t s
 // storage type (rows / planes need not be 16-byte aligned).
 template <typename ST> int flat_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 
+// chain kernels (gspn_chain_bwd.cu / gspn_chain_fwd.cu): one warp per scan chain, no block barrier on the
+// serial path, operands staged asynchronously by a producer warp; any H, W <= 128 and storage type.
+template <typename ST> int chain_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
+
 // merge (gspn_merge.cu)
 template <typename ST>
 int merge_launch(const ST* y_dirs, const float* m, ST* y, int D, int B, int C, int H, int W,
