@@ -28,7 +28,7 @@ template <> struct Elem<__nv_bfloat16> {
         return v;
     }
     static __device__ __forceinline__ void sts(uint32_t a, raw_t v) {
-        asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"(v) : "memory");
+        asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"(v));
     }
     static __device__ __forceinline__ float f(raw_t r) { return __uint_as_float(((uint32_t)r) << 16); }
     // fp32 = a*b + c with a, b storage values: one FHFMA.BF16
@@ -48,7 +48,7 @@ template <> struct Elem<float> {
         return v;
     }
     static __device__ __forceinline__ void sts(uint32_t a, raw_t v) {
-        asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory");
+        asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v));
     }
     static __device__ __forceinline__ float f(raw_t r) { return r; }
     static __device__ __forceinline__ float fma2(raw_t a, raw_t b, float c) { return fmaf(a, b, c); }

@@ -30,6 +30,7 @@
 namespace gspn {
 
 constexpr int kChMaxNS = 8;                       // channels per group the kernel takes
+constexpr int kChNPW = 4;                         // producer warps
 constexpr int kChMaxPlanes = 3 + 4 * kChMaxNS;    // w0 w1 w2, lambda[c], x[c], u[c], dy[c]
 constexpr int kTilePitch = 10;                    // elements per row of an 8-column output tile (odd word pitch)
 
@@ -49,10 +50,20 @@ struct ChainBwdParams {
 
 enum { KW0 = 0, KW1, KW2, KLAM, KX, KU, KDY, KNUM };
 
+__device__ __forceinline__ float maskf(float v, uint32_t m) { return __uint_as_float(__float_as_uint(v) & m); }
+__device__ __forceinline__ float lds32(uint32_t a) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v)); }
+
 // ---------------------------------------------------------------------------------------------------
 // One direction of one channel: the warp-level adjoint scan.  VH = false: T->B / B->T (lanes own
-// columns), true: L->R / R->L (lanes own rows).
-template <typename ST, int P, bool VH>
+// columns), true: L->R / R->L (lanes own rows); REV = the direction walks the image lines downwards.
+// Lane-dependent conditions (position inside the line, first / last position) are 32-bit AND masks in
+// ordinary registers, not predicates: values of positions past the line are forced to +0 exactly.
+template <typename ST, int P, bool VH, bool REV>
 __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* smem, const int d, const int b,
                                               const int g, const int c, const int lane, uint32_t& pf) {
     using E = Elem<ST>;
@@ -62,7 +73,6 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
     constexpr unsigned FULLM = 0xffffffffu;
     const Shape sh = p.sh;
     const int H = sh.H, W = sh.W, NS = p.NS;
-    const bool rev = d & 1;
     const int Ls = VH ? W : H, Lp = VH ? H : W, Lmax = sh.Lmax();
     const int NB = (Ls + kBlk - 1) / kBlk;
     const uint32_t rowB = (uint32_t)W * ES;
@@ -75,26 +85,37 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
     const int sidx[KNUM] = {0, 1, 2, 3 + c, 3 + NS + c, 3 + 2 * NS + c, 3 + 3 * NS + c};
 
     bool ok[P];
-#pragma unroll
-    for (int e = 0; e < P; ++e) ok[e] = P * lane + e < Lp;
+    uint32_t okm[P], m_w2[P];
     const int last_lane = (Lp - 1) / P, last_e = (Lp - 1) % P;
+#pragma unroll
+    for (int e = 0; e < P; ++e) {
+        ok[e] = P * lane + e < Lp;
+        okm[e] = ok[e] ? 0xffffffffu : 0u;
+        m_w2[e] = (lane == last_lane && e == last_e) ? 0u : 0xffffffffu;      // out-of-grid taps are never used
+    }
+    const uint32_t m_first = lane == 0 ? 0u : 0xffffffffu;
+    const uint32_t m_31 = lane == 31 ? 0u : 0xffffffffu;
 
     const size_t pc = ((size_t)qd * sh.B + b) * sh.C + (size_t)g * NS + c;    // plane in [D,B,C]
     const size_t pw = (((size_t)qd * sh.B + b) * sh.G + g) * 3;                // first tap plane in [D,B,G,3]
-    ST* du_g = p.du ? reinterpret_cast<ST*>(p.du) + pc * HW : nullptr;
-    ST* dlam_g = p.dlam ? reinterpret_cast<ST*>(p.dlam) + pc * HW : nullptr;
-    ST* dw_g = p.dw3 ? reinterpret_cast<ST*>(p.dw3) + pw * HW : nullptr;
-    float* DX = reinterpret_cast<float*>(smem + p.off_dx) + (size_t)c * H * p.Wp;
-    const bool want_dx = p.dx != nullptr;
-    float* ck = reinterpret_cast<float*>(smem + p.off_ckpt + (size_t)c * p.ckpt_warp);     // [NB][P][32]
-    float* exch = reinterpret_cast<float*>(smem + p.off_exch);                             // [NS][3][kBlk][P][32]
-    const uint32_t tile = smem_u32(smem + p.off_tile + (size_t)c * p.tile_warp);           // [2][Lp][kTilePitch]
-    const uint32_t dwtile = smem_u32(smem + p.off_dwtile);                                 // [3][Lp][kTilePitch]
+    const bool w_du = p.du != nullptr, w_dl = p.dlam != nullptr, w_dw = p.dw3 != nullptr, w_dx = p.dx != nullptr;
+    // this lane's first element of each output plane (vertical: column P*lane, horizontal: see the tile write-out)
+    ST* du_l = reinterpret_cast<ST*>(p.du) + pc * HW + (VH ? 0 : P * lane);
+    ST* dl_l = reinterpret_cast<ST*>(p.dlam) + pc * HW + (VH ? 0 : P * lane);
+    ST* dw_l = reinterpret_cast<ST*>(p.dw3) + pw * HW + (VH ? 0 : P * lane);
+    const uint32_t dxs = smem_u32(smem + p.off_dx) + (uint32_t)c * H * p.Wp * 4;               // this channel's fp32 dx plane
+    const uint32_t cks = smem_u32(smem + p.off_ckpt) + c * p.ckpt_warp + lane * 4;             // [NB][P][32]
+    const uint32_t exs = smem_u32(smem + p.off_exch) + lane * 4;                               // [NS][3][kBlk][P][32]
+    const uint32_t exw = exs + (uint32_t)c * 3 * kBlk * P * 128;
+    const uint32_t tile = smem_u32(smem + p.off_tile) + c * p.tile_warp;                       // [2][Lp][kTilePitch]
+    const uint32_t dwtile = smem_u32(smem + p.off_dwtile);                                     // [3][Lp][kTilePitch]
+    const uint32_t tplane = (uint32_t)Lp * kTilePitch * ES;
 
     // operand addresses inside the ring
     uint32_t phs[KNUM];          // vertical: byte phase (mod 16) of each plane
-    uint32_t vb[KNUM];           // vertical: per block, address of (local row 0, this lane's first column)
+    uint32_t vb[KNUM];           // vertical: per block, address of (local line 0, this lane's first column)
     uint32_t hb[KNUM][P];        // horizontal: address of (this lane's row e, chunk slot 0) + the row's byte phase
+    uint32_t dxh[P], tlh[P];     // horizontal: dx / tile row addresses of this lane's rows
     if constexpr (!VH) {
 #pragma unroll
         for (int k = 0; k < KNUM; ++k) { phs[k] = (uint32_t)(tb[sidx[k]].b0 & 15ull); vb[k] = 0; }
@@ -106,11 +127,17 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
             for (int k = 0; k < KNUM; ++k)
                 hb[k][e] = ring + sidx[k] * p.hplane + row * p.hrow +
                            (uint32_t)((tb[sidx[k]].b0 + (unsigned long long)row * rowB) % CB);
+            dxh[e] = dxs + (uint32_t)row * p.Wp * 4;
+            tlh[e] = tile + (uint32_t)row * kTilePitch * ES;
         }
     }
-    auto ldr = [&](int k, uint32_t boff, int e) -> raw_t {
-        if constexpr (!VH) return E::lds(vb[k] + boff + e * ES);
-        else return E::lds(hb[k][e] + boff);
+    // address of element e of operand k on image-local line tl of the current block
+    // (plain loads: the scheduler may hoist them over the asm stores of the previous step; the mbarrier
+    //  waits / arrives carry memory clobbers and keep them inside the stage's lifetime)
+    const uint8_t* const sbase = smem - smem_u32(smem);           // generic address of shared offset 0
+    auto ldr = [&](int k, int tl, uint32_t so, int e) -> raw_t {
+        if constexpr (!VH) return *reinterpret_cast<const raw_t*>(sbase + (vb[k] + tl * rowB + e * ES));
+        else return *reinterpret_cast<const raw_t*>(sbase + (hb[k][e] + so + tl * ES));
     };
 
     // ring hand-shake: block bi needs row block bi (vertical) / chunk columns bi and bi+1 (horizontal)
@@ -144,7 +171,7 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
             }
         }
     };
-    auto block_setup = [&](int bi) -> uint32_t {        // returns the block's base offset
+    auto block_setup = [&](int bi) -> uint32_t {        // returns the block's chunk-slot offset (horizontal)
         if constexpr (!VH) {
             const uint32_t stage = ring + (bi % p.NSV) * p.vstage;
             const uint32_t rb = ((uint32_t)(kBlk * bi) * rowB) & 15u;
@@ -156,32 +183,28 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
             return (uint32_t)(bi % p.NSH) * CB;
         }
     };
-    auto line_off = [&](uint32_t base, int tl) -> uint32_t { return VH ? base + tl * ES : base + tl * rowB; };
 
-    // one forward step: hout = w[s] hin + lambda[s]*x[s]
-    auto fwd_step = [&](const float (&hin)[P], uint32_t boff, float (&hout)[P]) {
+    // one forward step on image-local line tl: hout = w[s] hin + lambda[s]*x[s]
+    auto fwd_step = [&](const float (&hin)[P], int tl, uint32_t so, float (&hout)[P]) {
         raw_t w0r[P], w1r[P], w2r[P], lr[P], xr[P];
 #pragma unroll
         for (int e = 0; e < P; ++e) {
-            w0r[e] = ldr(KW0, boff, e); w1r[e] = ldr(KW1, boff, e); w2r[e] = ldr(KW2, boff, e);
-            lr[e] = ldr(KLAM, boff, e); xr[e] = ldr(KX, boff, e);
+            w0r[e] = ldr(KW0, tl, so, e); w1r[e] = ldr(KW1, tl, so, e); w2r[e] = ldr(KW2, tl, so, e);
+            lr[e] = ldr(KLAM, tl, so, e); xr[e] = ldr(KX, tl, so, e);
         }
-        float hl = __shfl_up_sync(FULLM, hin[P - 1], 1);
-        float hr = __shfl_down_sync(FULLM, hin[0], 1);
-        if (lane == 0) hl = 0.f;
-        if (lane == 31) hr = 0.f;
+        const float hl = maskf(__shfl_up_sync(FULLM, hin[P - 1], 1), m_first);
+        const float hr = __shfl_down_sync(FULLM, hin[0], 1);     // lane 31: masked through m_w2 / okm
 #pragma unroll
         for (int e = 0; e < P; ++e) {
-            float w0f = E::f(w0r[e]), w2f = E::f(w2r[e]);
-            if (e == 0 && lane == 0) w0f = 0.f;                         // out-of-grid taps are never used
-            if (lane == last_lane && e == last_e) w2f = 0.f;
+            const float w0f = e == 0 ? maskf(E::f(w0r[e]), m_first) : E::f(w0r[e]);
+            const float w2f = maskf(E::f(w2r[e]), m_w2[e]);
             const float left = e ? hin[e - 1] : hl;
             const float right = e < P - 1 ? hin[e + 1] : hr;
             float acc = E::f(w1r[e]) * hin[e];
             acc = fmaf(w0f, left, acc);
             acc = fmaf(w2f, right, acc);
             acc = E::fma2(lr[e], xr[e], acc);
-            hout[e] = ok[e] ? acc : 0.f;                                // positions past the line stay 0
+            hout[e] = maskf(acc, okm[e]);                               // positions past the line stay +0
         }
     };
 
@@ -192,29 +215,29 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
         h[e] = 0.f;
         if (p.h0 && ok[e]) h[e] = ld_f(reinterpret_cast<const ST*>(p.h0) + pc * Lmax + P * lane + e);
     }
-    begin_pass(rev);
+    begin_pass(REV);
     for (int n = 0; n < NB; ++n) {
-        const int bi = rev ? NB - 1 - n : n;
+        const int bi = REV ? NB - 1 - n : n;
         const int nb = min(kBlk, Ls - kBlk * bi);
-        acquire(bi, rev);
+        acquire(bi, REV);
 #pragma unroll
-        for (int e = 0; e < P; ++e) ck[(bi * P + e) * 32 + lane] = h[e];
-        const uint32_t base = block_setup(bi);
+        for (int e = 0; e < P; ++e) sts32(cks + (bi * P + e) * 128, h[e]);
+        const uint32_t so = block_setup(bi);
 #pragma unroll
         for (int t = 0; t < kBlk; ++t) {
-            if (t < nb) {
-                const int tl = rev ? nb - 1 - t : t;
+            const int tl = REV ? kBlk - 1 - t : t;
+            if (tl < nb) {
                 float hn[P];
-                fwd_step(h, line_off(base, tl), hn);
+                fwd_step(h, tl, so, hn);
 #pragma unroll
                 for (int e = 0; e < P; ++e) h[e] = hn[e];
             }
         }
-        release(bi, rev, n == NB - 1);
+        release(bi, REV, n == NB - 1);
     }
 
     // ================= pass 2: reverse order ===========================================================
-    const bool desc2 = !rev;
+    constexpr bool desc2 = !REV;
     float carry[P];
 #pragma unroll
     for (int e = 0; e < P; ++e) carry[e] = 0.f;
@@ -223,125 +246,115 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
         const int bi = desc2 ? NB - 1 - n : n;
         const int nb = min(kBlk, Ls - kBlk * bi);
         acquire(bi, desc2);
-        const uint32_t base = block_setup(bi);
-        float hs[kBlk + 1][P];                  // hs[t] = state entering scan-local step t of the block
+        const uint32_t so = block_setup(bi);
+        float hs[kBlk + 1][P];                  // hs[t] = state entering the t-th step (scan order) of the block
 #pragma unroll
-        for (int e = 0; e < P; ++e) hs[0][e] = ck[(bi * P + e) * 32 + lane];
+        for (int e = 0; e < P; ++e) hs[0][e] = lds32(cks + (bi * P + e) * 128);
 #pragma unroll
         for (int t = 0; t < kBlk; ++t) {
-            if (t < nb) {
-                const int tl = rev ? nb - 1 - t : t;
-                fwd_step(hs[t], line_off(base, tl), hs[t + 1]);
+            const int tl = REV ? kBlk - 1 - t : t;
+            if (tl < nb) {
+                fwd_step(hs[t], tl, so, hs[t + 1]);
             } else {
 #pragma unroll
-                for (int e = 0; e < P; ++e) hs[t + 1][e] = 0.f;
+                for (int e = 0; e < P; ++e) hs[t + 1][e] = hs[t][e];
             }
+        }
+        // per-block output / accumulator addresses
+        const int l0 = kBlk * bi;                                   // first image line of the block
+        uint32_t dxv = 0, thb = 0;
+        ST *du_b = nullptr, *dl_b = nullptr;
+        if constexpr (!VH) {
+            dxv = dxs + ((uint32_t)l0 * p.Wp + P * lane) * 4;
+            du_b = du_l + (size_t)l0 * W;
+            dl_b = dl_l + (size_t)l0 * W;
+        } else {
+            thb = (uint32_t)((bi & 1) * kBlk) * ES;
         }
 #pragma unroll
         for (int tt = 0; tt < kBlk; ++tt) {
             const int t = kBlk - 1 - tt;
-            if (t < nb) {
-                const int tl = rev ? nb - 1 - t : t;
-                const int li = kBlk * bi + tl;                      // image line (row / column) of this step
-                const uint32_t boff = line_off(base, tl);
+            const int tl = REV ? kBlk - 1 - t : t;
+            if (tl < nb) {
                 raw_t w0r[P], w1r[P], w2r[P], lr[P], xr[P], ur[P], dyr[P];
 #pragma unroll
                 for (int e = 0; e < P; ++e) {
-                    ur[e] = ldr(KU, boff, e); dyr[e] = ldr(KDY, boff, e);
-                    lr[e] = ldr(KLAM, boff, e); xr[e] = ldr(KX, boff, e);
-                    w0r[e] = ldr(KW0, boff, e); w1r[e] = ldr(KW1, boff, e); w2r[e] = ldr(KW2, boff, e);
+                    ur[e] = ldr(KU, tl, so, e); dyr[e] = ldr(KDY, tl, so, e);
+                    lr[e] = ldr(KLAM, tl, so, e); xr[e] = ldr(KX, tl, so, e);
+                    w0r[e] = ldr(KW0, tl, so, e); w1r[e] = ldr(KW1, tl, so, e); w2r[e] = ldr(KW2, tl, so, e);
                 }
                 float gh[P];
 #pragma unroll
-                for (int e = 0; e < P; ++e) {
-                    const float v = E::fma2(dyr[e], ur[e], carry[e]);
-                    gh[e] = ok[e] ? v : 0.f;
-                }
-                // du, dlambda, dx
+                for (int e = 0; e < P; ++e) gh[e] = maskf(E::fma2(dyr[e], ur[e], carry[e]), okm[e]);
+                // du, dlambda
 #pragma unroll
                 for (int e = 0; e < P; ++e) {
-                    const float duv = E::f(dyr[e]) * hs[t + 1][e];
-                    const float dlv = E::f(xr[e]) * gh[e];
+                    const raw_t duv = E::pack(E::f(dyr[e]) * hs[t + 1][e]);
+                    const raw_t dlv = E::pack(E::f(xr[e]) * gh[e]);
                     if constexpr (!VH) {
-                        const size_t o = (size_t)li * W + P * lane + e;
-                        if (ok[e]) {
-                            if (du_g) E::stg(du_g + o, E::pack(duv));
-                            if (dlam_g) E::stg(dlam_g + o, E::pack(dlv));
-                            if (want_dx) {
-                                float* a = DX + li * p.Wp + P * lane + e;
-                                *a = fmaf(E::f(lr[e]), gh[e], *a);
-                            }
-                        }
+                        if (w_du && ok[e]) E::stg(du_b + tl * W + e, duv);
+                        if (w_dl && ok[e]) E::stg(dl_b + tl * W + e, dlv);
                     } else {
-                        const int row = P * lane + e;
-                        const int cs = (bi & 1) * kBlk + tl;
-                        if (ok[e]) {
-                            if (du_g) E::sts(tile + (row * kTilePitch + cs) * ES, E::pack(duv));
-                            if (dlam_g) E::sts(tile + ((Lp + row) * kTilePitch + cs) * ES, E::pack(dlv));
-                            if (want_dx) {
-                                float* a = DX + row * p.Wp + li;
-                                *a = fmaf(E::f(lr[e]), gh[e], *a);
-                            }
-                        }
+                        if (w_du && ok[e]) E::sts(tlh[e] + thb + tl * ES, duv);
+                        if (w_dl && ok[e]) E::sts(tlh[e] + tplane + thb + tl * ES, dlv);
+                    }
+                }
+                // dx += lambda * gh
+                if (w_dx) {
+#pragma unroll
+                    for (int e = 0; e < P; ++e) {
+                        const uint32_t a = VH ? dxh[e] + (l0 + tl) * 4 : dxv + (tl * p.Wp + e) * 4;
+                        if (ok[e]) sts32(a, fmaf(E::f(lr[e]), gh[e], lds32(a)));
                     }
                 }
                 // dw3 partials of this channel: gh * h[s-1, p+k-1]
-                if (dw_g) {
-                    float hpl = __shfl_up_sync(FULLM, hs[t][P - 1], 1);
-                    float hpr = __shfl_down_sync(FULLM, hs[t][0], 1);
-                    if (lane == 0) hpl = 0.f;
-                    if (lane == 31) hpr = 0.f;
+                if (w_dw) {
+                    const float hpl = maskf(__shfl_up_sync(FULLM, hs[t][P - 1], 1), m_first);
+                    const float hpr = maskf(__shfl_down_sync(FULLM, hs[t][0], 1), m_31);
 #pragma unroll
                     for (int e = 0; e < P; ++e) {
                         const float left = e ? hs[t][e - 1] : hpl;
                         const float right = e < P - 1 ? hs[t][e + 1] : hpr;
-                        float* x0 = exch + ((((size_t)c * 3 + 0) * kBlk + tl) * P + e) * 32 + lane;
-                        x0[0] = gh[e] * left;
-                        x0[(size_t)kBlk * P * 32] = gh[e] * hs[t][e];
-                        x0[(size_t)2 * kBlk * P * 32] = gh[e] * right;
+                        const uint32_t a = exw + (tl * P + e) * 128;
+                        sts32(a, gh[e] * left);
+                        sts32(a + kBlk * P * 128, gh[e] * hs[t][e]);
+                        sts32(a + 2 * kBlk * P * 128, gh[e] * right);
                     }
                 }
                 // carry = w[s]^T gh: position p receives from p-1 (its tap k=2), p (k=1), p+1 (k=0)
                 float a2[P], c0[P];
 #pragma unroll
                 for (int e = 0; e < P; ++e) {
-                    float w0f = E::f(w0r[e]), w2f = E::f(w2r[e]);
-                    if (e == 0 && lane == 0) w0f = 0.f;
-                    if (lane == last_lane && e == last_e) w2f = 0.f;
-                    a2[e] = w2f * gh[e];
+                    const float w0f = e == 0 ? maskf(E::f(w0r[e]), m_first) : E::f(w0r[e]);
+                    a2[e] = maskf(E::f(w2r[e]), m_w2[e]) * gh[e];
                     c0[e] = w0f * gh[e];
                 }
-                float al = __shfl_up_sync(FULLM, a2[P - 1], 1);
-                float cr = __shfl_down_sync(FULLM, c0[0], 1);
-                if (lane == 0) al = 0.f;
-                if (lane == 31) cr = 0.f;
+                const float al = maskf(__shfl_up_sync(FULLM, a2[P - 1], 1), m_first);
+                const float cr = maskf(__shfl_down_sync(FULLM, c0[0], 1), m_31);
 #pragma unroll
                 for (int e = 0; e < P; ++e) {
-                    float acc = E::f(w1r[e]) * gh[e];
-                    acc += e ? a2[e - 1] : al;
+                    float acc = fmaf(E::f(w1r[e]), gh[e], e ? a2[e - 1] : al);
                     acc += e < P - 1 ? c0[e + 1] : cr;
                     carry[e] = acc;
                 }
             }
         }
         // dw3 of the block: sum over the group's channels in ascending order, one RNE
-        if (dw_g) {
+        if (w_dw) {
             if (NS > 1) chain_bar(NS * 32); else __syncwarp();
             for (int kt = c; kt < 3 * kBlk; kt += NS) {
                 const int k = kt / kBlk, tl = kt % kBlk;
                 if (tl < nb) {
 #pragma unroll
                     for (int e = 0; e < P; ++e) {
-                        const float* x0 = exch + (((size_t)k * kBlk + tl) * P + e) * 32 + lane;
-                        float sum = x0[0];
-                        for (int s = 1; s < NS; ++s) sum += x0[(size_t)s * 3 * kBlk * P * 32];
-                        if (ok[e]) {
-                            if constexpr (!VH) {
-                                E::stg(dw_g + (size_t)k * HW + (size_t)(kBlk * bi + tl) * W + P * lane + e, E::pack(sum));
-                            } else {
-                                const int row = P * lane + e, cs = (bi & 1) * kBlk + tl;
-                                E::sts(dwtile + ((k * Lp + row) * kTilePitch + cs) * ES, E::pack(sum));
-                            }
+                        const uint32_t a = exs + ((k * kBlk + tl) * P + e) * 128;
+                        float sum = lds32(a);
+                        for (int s = 1; s < NS; ++s) sum += lds32(a + s * (3 * kBlk * P * 128));
+                        if constexpr (!VH) {
+                            if (ok[e]) E::stg(dw_l + (size_t)k * HW + (size_t)(l0 + tl) * W + e, E::pack(sum));
+                        } else {
+                            const int row = P * lane + e;
+                            if (ok[e]) E::sts(dwtile + ((k * Lp + row) * kTilePitch) * ES + thb + tl * ES, E::pack(sum));
                         }
                     }
                 }
@@ -354,17 +367,27 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
             if (pair_done) {
                 const int col0 = 2 * kBlk * (bi >> 1);
                 const int ncols = min(2 * kBlk, W - col0);
+                const int col = lane & 7, rsub = lane >> 3;
                 __syncwarp();
-                for (int idx = lane; idx < Lp * 2 * kBlk; idx += 32) {
-                    const int row = idx >> 3, col = idx & 7;
-                    if (col < ncols) {
-                        const size_t o = (size_t)row * W + col0 + col;
-                        if (du_g) E::stg(du_g + o, E::lds(tile + (row * kTilePitch + col) * ES));
-                        if (dlam_g) E::stg(dlam_g + o, E::lds(tile + ((Lp + row) * kTilePitch + col) * ES));
-                        if (dw_g)
-                            for (int k = c; k < 3; k += NS)
-                                E::stg(dw_g + (size_t)k * HW + o, E::lds(dwtile + ((k * Lp + row) * kTilePitch + col) * ES));
+                if (col < ncols) {
+                    uint32_t ta = tile + (rsub * kTilePitch + col) * ES;
+                    const size_t o = (size_t)rsub * W + col0 + col;
+                    ST* g0 = du_l + o;
+                    ST* g1 = dl_l + o;
+                    for (int r = rsub; r < Lp; r += 4) {
+                        if (w_du) E::stg(g0, E::lds(ta));
+                        if (w_dl) E::stg(g1, E::lds(ta + tplane));
+                        ta += 4 * kTilePitch * ES; g0 += 4 * W; g1 += 4 * W;
                     }
+                    if (w_dw)
+                        for (int k = c; k < 3; k += NS) {
+                            uint32_t tw = dwtile + ((k * Lp + rsub) * kTilePitch + col) * ES;
+                            ST* g2 = dw_l + (size_t)k * HW + o;
+                            for (int r = rsub; r < Lp; r += 4) {
+                                E::stg(g2, E::lds(tw));
+                                tw += 4 * kTilePitch * ES; g2 += 4 * W;
+                            }
+                        }
                 }
                 __syncwarp();
             }
@@ -383,7 +406,7 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
 
 // ---------------------------------------------------------------------------------------------------
 template <typename ST, int P>
-__global__ void __launch_bounds__(32 * (1 + kChMaxNS), 1)
+__global__ void __launch_bounds__(32 * (kChNPW + kChMaxNS), 1)
 chain_bwd_kernel(const ChainBwdParams p) {
     constexpr int ES = sizeof(ST);
     constexpr int CB = kBlk * ES;
@@ -425,18 +448,23 @@ chain_bwd_kernel(const ChainBwdParams p) {
         }
     }
     if (threadIdx.x == 0) {
-        for (int s = 0; s < kChSlots; ++s) { mbar_init(&full[s], 33); mbar_init(&empty[s], NS); }
+        for (int s = 0; s < kChSlots; ++s) { mbar_init(&full[s], kChNPW * 33); mbar_init(&empty[s], NS); }
         mbar_init_fence();
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // zeros (generic proxy) before bulk copies
     __syncthreads();
 
-    if (warp == 0) {
-        // ---------------- producer ------------------------------------------------------------------
+    if (warp < kChNPW) {
+        // ---------------- producer warp pw: planes pw, pw + NPW, ... of every stage ----------------------
+        const int pw = warp;
         const uint32_t ring = smem_u32(smem + p.off_ring);
         uint8_t* ringp = smem + p.off_ring;
         uint32_t pe = 0;
         bool drained = false;
+        // horizontal: this lane copies rows lane, lane+32, ... of each of its planes
+        uint32_t rowoff[4], rowdst[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) { rowoff[r] = (uint32_t)(lane + 32 * r) * rowB; rowdst[r] = (uint32_t)(lane + 32 * r) * p.hrow; }
         for (int d = 0; d < 4; ++d) {
             if (p.q[d] < 0) continue;
             const bool vh = d >> 1, rev = d & 1;
@@ -452,6 +480,9 @@ chain_bwd_kernel(const ChainBwdParams p) {
                 const bool desc = rev != (pass == 1);
                 if (!vh) {
                     const int NB = (H + kBlk - 1) / kBlk;
+                    const int s = lane * kChNPW + pw;                 // this lane's plane
+                    ChPlane e{nullptr, 0, 0};
+                    if (s < npp) e = tb[s];
                     for (int n = 0; n < NB; ++n) {
                         const int bi = desc ? NB - 1 - n : n;
                         const int slot = bi % p.NSV;
@@ -459,37 +490,26 @@ chain_bwd_kernel(const ChainBwdParams p) {
                         mbar_wait(&empty[slot], ((pe >> slot) & 1u) ^ 1u);
                         pe ^= 1u << slot;
                         uint64_t* fb = &full[slot];
-                        int nbytes[2] = {0, 0};
-                        unsigned long long a0[2] = {0, 0};
-#pragma unroll
-                        for (int r = 0; r < 2; ++r) {
-                            const int s = lane + 32 * r;
-                            if (s < npp) {
-                                const ChPlane e = tb[s];
-                                uint8_t* dst = ringp + (size_t)slot * p.vstage + (size_t)s * p.vslot;
-                                const unsigned long long byte0 = e.b0 + (unsigned long long)r0 * rowB;
-                                const unsigned long long byte1 = e.b0 + (unsigned long long)r1 * rowB;
-                                a0[r] = byte0 & ~15ull;
-                                const unsigned long long lim = e.tbytes & ~15ull;
-                                unsigned long long a1 = (byte1 + 15) & ~15ull;
-                                if (a1 > lim) a1 = lim;
-                                nbytes[r] = a1 > a0[r] ? (int)(a1 - a0[r]) : 0;
-                                if (byte1 > a1)      // bytes past the tensor's last whole 16-byte chunk: ordinary loads
-                                    for (unsigned long long o = (a1 > byte0 ? a1 : byte0); o < byte1; o += ES)
-                                        *reinterpret_cast<ST*>(dst + (o - a0[r])) = *reinterpret_cast<const ST*>(e.base + o);
-                            }
+                        int nbytes = 0;
+                        unsigned long long a0 = 0;
+                        uint8_t* dst = ringp + (size_t)slot * p.vstage + (size_t)s * p.vslot;
+                        if (s < npp) {
+                            const unsigned long long byte0 = e.b0 + (unsigned long long)r0 * rowB;
+                            const unsigned long long byte1 = e.b0 + (unsigned long long)r1 * rowB;
+                            a0 = byte0 & ~15ull;
+                            const unsigned long long lim = e.tbytes & ~15ull;
+                            unsigned long long a1 = (byte1 + 15) & ~15ull;
+                            if (a1 > lim) a1 = lim;
+                            nbytes = a1 > a0 ? (int)(a1 - a0) : 0;
+                            if (byte1 > a1)      // bytes past the tensor's last whole 16-byte chunk: ordinary loads
+                                for (unsigned long long o = (a1 > byte0 ? a1 : byte0); o < byte1; o += ES)
+                                    *reinterpret_cast<ST*>(dst + (o - a0)) = *reinterpret_cast<const ST*>(e.base + o);
                         }
-                        const int total = warp_sum(nbytes[0] + nbytes[1]);
+                        const int total = warp_sum(nbytes);
                         __syncwarp();
                         if (lane == 0) mbar_arrive_expect_tx(fb, (uint32_t)total);
                         __syncwarp();
-#pragma unroll
-                        for (int r = 0; r < 2; ++r) {
-                            const int s = lane + 32 * r;
-                            if (s < npp && nbytes[r] > 0)
-                                bulk_load_1d(ringp + (size_t)slot * p.vstage + (size_t)s * p.vslot, tb[s].base + a0[r],
-                                             (uint32_t)nbytes[r], fb);
-                        }
+                        if (nbytes > 0) bulk_load_1d(dst, e.base + a0, (uint32_t)nbytes, fb);
                         mbar_arrive(fb);
                     }
                 } else {
@@ -499,26 +519,30 @@ chain_bwd_kernel(const ChainBwdParams p) {
                         mbar_wait(&empty[slot], ((pe >> slot) & 1u) ^ 1u);
                         pe ^= 1u << slot;
                         uint64_t* fb = &full[slot];
-                        int s = 0, i = lane;
-                        while (i >= H) { i -= H; ++s; }
-                        while (s < npp) {
+                        const unsigned long long qoff = (unsigned long long)qn * CB;
+                        for (int s = pw; s < npp; s += kChNPW) {
                             const ChPlane e = tb[s];
-                            const unsigned long long rowb = e.b0 + (unsigned long long)i * rowB;
-                            const unsigned long long cb = (rowb / CB + qn) * CB;
-                            const uint32_t dst = ring + s * p.hplane + i * p.hrow + slot * CB;
-                            if (cb + CB <= e.tbytes) {
-                                cp_async_cb<CB>(dst, e.base + cb);
-                                if (slot == 0) cp_async_cb<CB>(dst + p.NSH * CB, e.base + cb);
-                            } else if (cb < e.tbytes) {
-                                uint8_t* dp = ringp + (size_t)s * p.hplane + (size_t)i * p.hrow + (size_t)slot * CB;
-                                for (unsigned long long o = cb; o < e.tbytes; o += ES) {
-                                    const ST v = *reinterpret_cast<const ST*>(e.base + o);
-                                    *reinterpret_cast<ST*>(dp + (o - cb)) = v;
-                                    if (slot == 0) *reinterpret_cast<ST*>(dp + p.NSH * CB + (o - cb)) = v;
+                            const uint32_t dpl = ring + s * p.hplane + slot * CB;
+                            // every chunk this plane can ask for lies inside the tensor: no per-chunk bound checks
+                            const bool safe = e.b0 + HW * ES + (unsigned long long)(p.NQ + 1) * CB <= e.tbytes;
+#pragma unroll
+                            for (int r = 0; r < 4; ++r) {
+                                if (lane + 32 * r < H) {
+                                    const unsigned long long cb = ((e.b0 + rowoff[r]) & ~(unsigned long long)(CB - 1)) + qoff;
+                                    const uint32_t dst = dpl + rowdst[r];
+                                    if (safe || cb + CB <= e.tbytes) {
+                                        cp_async_cb<CB>(dst, e.base + cb);
+                                        if (slot == 0) cp_async_cb<CB>(dst + p.NSH * CB, e.base + cb);
+                                    } else if (cb < e.tbytes) {
+                                        uint8_t* dp = ringp + (dst - ring);
+                                        for (unsigned long long o = cb; o < e.tbytes; o += ES) {
+                                            const ST v = *reinterpret_cast<const ST*>(e.base + o);
+                                            *reinterpret_cast<ST*>(dp + (o - cb)) = v;
+                                            if (slot == 0) *reinterpret_cast<ST*>(dp + p.NSH * CB + (o - cb)) = v;
+                                        }
+                                    }
                                 }
                             }
-                            i += 32;
-                            while (i >= H) { i -= H; ++s; }
                         }
                         cp_async_arrive_noinc(fb);
                         __syncwarp();
@@ -527,15 +551,14 @@ chain_bwd_kernel(const ChainBwdParams p) {
                 }
             }
         }
-    } else if (warp <= NS) {
+    } else if (warp < kChNPW + NS) {
         // ---------------- chain warp of channel c ------------------------------------------------------
-        const int c = warp - 1;
+        const int c = warp - kChNPW;
         uint32_t pf = 0;
-        for (int d = 0; d < 4; ++d) {
-            if (p.q[d] < 0) continue;
-            if (d < 2) chain_bwd_dir<ST, P, false>(p, smem, d, b, g, c, lane, pf);
-            else       chain_bwd_dir<ST, P, true>(p, smem, d, b, g, c, lane, pf);
-        }
+        if (p.q[0] >= 0) chain_bwd_dir<ST, P, false, false>(p, smem, 0, b, g, c, lane, pf);
+        if (p.q[1] >= 0) chain_bwd_dir<ST, P, false, true>(p, smem, 1, b, g, c, lane, pf);
+        if (p.q[2] >= 0) chain_bwd_dir<ST, P, true, false>(p, smem, 2, b, g, c, lane, pf);
+        if (p.q[3] >= 0) chain_bwd_dir<ST, P, true, true>(p, smem, 3, b, g, c, lane, pf);
     }
     __syncthreads();
 
@@ -633,7 +656,7 @@ int chain_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li) {
     prm.bytes_w = (unsigned long long)sh.D() * sh.B * sh.G * 3 * sh.H * sh.W * ES;
     int q = 0;
     for (int d = 0; d < 4; ++d) prm.q[d] = (sh.mask >> d & 1u) ? q++ : -1;
-    const int threads = 32 * (1 + NS), items = sh.B * sh.G;
+    const int threads = 32 * (kChNPW + NS), items = sh.B * sh.G;
     int rc = GSPN_EUNSUPPORTED;
     switch (P) {
     case 1: rc = launch_chain_bwd<ST, 1>(prm, items, threads, st); break;
