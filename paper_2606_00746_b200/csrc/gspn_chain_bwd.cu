@@ -29,7 +29,9 @@
 
 namespace gspn {
 
-constexpr int kChMaxNS = 8;                       // channels per group the kernel takes
+constexpr int kChMaxNS = 4;                       // channels per group the kernel takes
+constexpr int kChNO = kBlk;                       // output warps: one per step of a block
+constexpr int kChBars = 2 * kChSlots + 4;         // full[8] empty[8] ready[2] free[2]
 constexpr int kChNPW = 4;                         // producer warps
 constexpr int kChMaxPlanes = 3 + 4 * kChMaxNS;    // w0 w1 w2, lambda[c], x[c], u[c], dy[c]
 constexpr int kTilePitch = 10;                    // elements per row of an 8-column output tile (odd word pitch)
@@ -42,8 +44,8 @@ struct ChainBwdParams {
     int NSV, NSH, NQ;               // ring slots (row blocks / chunk columns); chunk columns per row
     int Wp;                         // row pitch of the dx planes in floats
     uint32_t vslot, vstage, hrow, hplane;
-    uint32_t off_tab, off_dx, off_ring, off_ckpt, off_exch, off_tile, off_dwtile, total;
-    uint32_t ckpt_warp, tile_warp;  // bytes per chain warp
+    uint32_t off_tab, off_dx, off_ring, off_ckpt, off_hb, off_gb, off_tile, total;
+    uint32_t ckpt_warp;             // checkpoint bytes per channel
     int q[4];                       // slab index of each direction, -1 = not in dir_mask
     unsigned long long bytes_x, bytes_c, bytes_w;
 };
@@ -59,13 +61,71 @@ __device__ __forceinline__ float lds32(uint32_t a) {
 __device__ __forceinline__ void sts32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v)); }
 
 // ---------------------------------------------------------------------------------------------------
-// One direction of one channel: the warp-level adjoint scan.  VH = false: T->B / B->T (lanes own
-// columns), true: L->R / R->L (lanes own rows); REV = the direction walks the image lines downwards.
+// Ring hand-shake of a consumer warp.  Block bi (image lines [4bi, 4bi+4)) needs row block bi
+// (vertical) or chunk columns bi and bi+1 (horizontal).  Every consumer warp of the CTA acquires and
+// releases every stage, whether its role has work in it or not, so the mbarrier phases stay aligned.
+template <bool VH>
+struct RingSync {
+    uint64_t *full, *empty;
+    int NSV, NSH, NQ, lane, hq;
+    uint32_t pf;
+    __device__ __forceinline__ void wait_full(int slot) {
+        mbar_wait(&full[slot], (pf >> slot) & 1u);
+        pf ^= 1u << slot;
+    }
+    __device__ __forceinline__ void begin_pass(bool desc) { hq = desc ? NQ - 1 : 0; }
+    __device__ __forceinline__ void acquire(int bi, bool desc) {
+        if constexpr (!VH) {
+            wait_full(bi % NSV);
+        } else if (!desc) {
+            const int need = min(bi + 1, NQ - 1);
+            for (; hq <= need; ++hq) wait_full(hq % NSH);
+        } else {
+            for (; hq >= bi; --hq) wait_full(hq % NSH);
+        }
+    }
+    __device__ __forceinline__ void release(int bi, bool desc, bool last) {
+        __syncwarp();
+        if (lane == 0) {
+            if constexpr (!VH) {
+                mbar_arrive(&empty[bi % NSV]);
+            } else if (!desc) {
+                mbar_arrive(&empty[bi % NSH]);
+                if (last) for (int qq = bi + 1; qq < NQ; ++qq) mbar_arrive(&empty[qq % NSH]);
+            } else {
+                if (bi + 1 < NQ) mbar_arrive(&empty[(bi + 1) % NSH]);
+                if (last) mbar_arrive(&empty[bi % NSH]);
+            }
+        }
+    }
+};
+
+// hand-over of one block's h / gh lines from the chain warps to the output warps (double buffered)
+struct BlockSync {
+    uint64_t *ready, *freeb;      // [2] each
+    uint32_t n;                   // blocks handed over so far (all directions)
+    __device__ __forceinline__ int buf() const { return n & 1u; }
+    __device__ __forceinline__ void producer_wait() { mbar_wait(&freeb[n & 1u], ((n >> 1) & 1u) ^ 1u); }
+    __device__ __forceinline__ void producer_done(int lane) { __syncwarp(); if (lane == 0) mbar_arrive(&ready[n & 1u]); ++n; }
+    __device__ __forceinline__ void consumer_wait() { mbar_wait(&ready[n & 1u], (n >> 1) & 1u); }
+    __device__ __forceinline__ void consumer_done(int lane) { __syncwarp(); if (lane == 0) mbar_arrive(&freeb[n & 1u]); ++n; }
+};
+
+// ---------------------------------------------------------------------------------------------------
+// Chain warps of channel c, one direction.  VH = false: T->B / B->T (lanes own columns), true:
+// L->R / R->L (lanes own rows); REV = the direction walks the image lines downwards.
+//   ROLE_A  pass 1: h[s] = w[s] h[s-1] + lambda[s]*x[s] in scan order, the state entering every block
+//                   stored as a checkpoint; pass 2: the adjoint chain gh[s] = dy[s]*u[s] + w[s+1]^T gh[s+1]
+//                   in reverse order, gh of every step handed to the output warps; dh0 at the end.
+//   ROLE_F  pass 2: h of the block's steps recomputed from its checkpoint, handed to the output warps.
 // Lane-dependent conditions (position inside the line, first / last position) are 32-bit AND masks in
-// ordinary registers, not predicates: values of positions past the line are forced to +0 exactly.
-template <typename ST, int P, bool VH, bool REV>
+// ordinary registers: values of positions past the line are forced to +0 exactly.
+enum { ROLE_A = 0, ROLE_F = 1 };
+
+template <typename ST, int P, bool VH, bool REV, int ROLE>
 __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* smem, const int d, const int b,
-                                              const int g, const int c, const int lane, uint32_t& pf) {
+                                              const int g, const int c, const int lane, uint32_t& pf,
+                                              BlockSync& bs) {
     using E = Elem<ST>;
     using raw_t = typename E::raw_t;
     constexpr int ES = sizeof(ST);
@@ -77,12 +137,11 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
     const int NB = (Ls + kBlk - 1) / kBlk;
     const uint32_t rowB = (uint32_t)W * ES;
     const int qd = p.q[d];
-    const size_t HW = (size_t)H * W;
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem);
-    uint64_t* empty = full + kChSlots;
     const ChPlane* tb = reinterpret_cast<const ChPlane*>(smem + p.off_tab) + d * kChMaxPlanes;
     const uint32_t ring = smem_u32(smem + p.off_ring);
     const int sidx[KNUM] = {0, 1, 2, 3 + c, 3 + NS + c, 3 + 2 * NS + c, 3 + 3 * NS + c};
+    RingSync<VH> rs{reinterpret_cast<uint64_t*>(smem), reinterpret_cast<uint64_t*>(smem) + kChSlots,
+                    p.NSV, p.NSH, p.NQ, lane, 0, pf};
 
     bool ok[P];
     uint32_t okm[P], m_w2[P];
@@ -97,25 +156,14 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
     const uint32_t m_31 = lane == 31 ? 0u : 0xffffffffu;
 
     const size_t pc = ((size_t)qd * sh.B + b) * sh.C + (size_t)g * NS + c;    // plane in [D,B,C]
-    const size_t pw = (((size_t)qd * sh.B + b) * sh.G + g) * 3;                // first tap plane in [D,B,G,3]
-    const bool w_du = p.du != nullptr, w_dl = p.dlam != nullptr, w_dw = p.dw3 != nullptr, w_dx = p.dx != nullptr;
-    // this lane's first element of each output plane (vertical: column P*lane, horizontal: see the tile write-out)
-    ST* du_l = reinterpret_cast<ST*>(p.du) + pc * HW + (VH ? 0 : P * lane);
-    ST* dl_l = reinterpret_cast<ST*>(p.dlam) + pc * HW + (VH ? 0 : P * lane);
-    ST* dw_l = reinterpret_cast<ST*>(p.dw3) + pw * HW + (VH ? 0 : P * lane);
-    const uint32_t dxs = smem_u32(smem + p.off_dx) + (uint32_t)c * H * p.Wp * 4;               // this channel's fp32 dx plane
     const uint32_t cks = smem_u32(smem + p.off_ckpt) + c * p.ckpt_warp + lane * 4;             // [NB][P][32]
-    const uint32_t exs = smem_u32(smem + p.off_exch) + lane * 4;                               // [NS][3][kBlk][P][32]
-    const uint32_t exw = exs + (uint32_t)c * 3 * kBlk * P * 128;
-    const uint32_t tile = smem_u32(smem + p.off_tile) + c * p.tile_warp;                       // [2][Lp][kTilePitch]
-    const uint32_t dwtile = smem_u32(smem + p.off_dwtile);                                     // [3][Lp][kTilePitch]
-    const uint32_t tplane = (uint32_t)Lp * kTilePitch * ES;
+    const uint32_t hbuf = smem_u32(smem + p.off_hb) + (uint32_t)c * 2 * (kBlk + 1) * P * 128 + lane * 4;  // [2][kBlk+1][P][32]
+    const uint32_t gbuf = smem_u32(smem + p.off_gb) + (uint32_t)c * 2 * kBlk * P * 128 + lane * 4;        // [2][kBlk][P][32]
 
     // operand addresses inside the ring
     uint32_t phs[KNUM];          // vertical: byte phase (mod 16) of each plane
     uint32_t vb[KNUM];           // vertical: per block, address of (local line 0, this lane's first column)
     uint32_t hb[KNUM][P];        // horizontal: address of (this lane's row e, chunk slot 0) + the row's byte phase
-    uint32_t dxh[P], tlh[P];     // horizontal: dx / tile row addresses of this lane's rows
     if constexpr (!VH) {
 #pragma unroll
         for (int k = 0; k < KNUM; ++k) { phs[k] = (uint32_t)(tb[sidx[k]].b0 & 15ull); vb[k] = 0; }
@@ -127,49 +175,14 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
             for (int k = 0; k < KNUM; ++k)
                 hb[k][e] = ring + sidx[k] * p.hplane + row * p.hrow +
                            (uint32_t)((tb[sidx[k]].b0 + (unsigned long long)row * rowB) % CB);
-            dxh[e] = dxs + (uint32_t)row * p.Wp * 4;
-            tlh[e] = tile + (uint32_t)row * kTilePitch * ES;
         }
     }
-    // address of element e of operand k on image-local line tl of the current block
-    // (plain loads: the scheduler may hoist them over the asm stores of the previous step; the mbarrier
-    //  waits / arrives carry memory clobbers and keep them inside the stage's lifetime)
+    // element e of operand k on image-local line tl of the current block (plain loads: the mbarrier
+    // waits / arrives carry memory clobbers and keep them inside the stage's lifetime)
     const uint8_t* const sbase = smem - smem_u32(smem);           // generic address of shared offset 0
     auto ldr = [&](int k, int tl, uint32_t so, int e) -> raw_t {
         if constexpr (!VH) return *reinterpret_cast<const raw_t*>(sbase + (vb[k] + tl * rowB + e * ES));
         else return *reinterpret_cast<const raw_t*>(sbase + (hb[k][e] + so + tl * ES));
-    };
-
-    // ring hand-shake: block bi needs row block bi (vertical) / chunk columns bi and bi+1 (horizontal)
-    int hq = 0;
-    auto wait_full = [&](int slot) {
-        mbar_wait(&full[slot], (pf >> slot) & 1u);
-        pf ^= 1u << slot;
-    };
-    auto begin_pass = [&](bool desc) { hq = desc ? p.NQ - 1 : 0; };
-    auto acquire = [&](int bi, bool desc) {
-        if constexpr (!VH) {
-            wait_full(bi % p.NSV);
-        } else if (!desc) {
-            const int need = min(bi + 1, p.NQ - 1);
-            for (; hq <= need; ++hq) wait_full(hq % p.NSH);
-        } else {
-            for (; hq >= bi; --hq) wait_full(hq % p.NSH);
-        }
-    };
-    auto release = [&](int bi, bool desc, bool last) {
-        __syncwarp();
-        if (lane == 0) {
-            if constexpr (!VH) {
-                mbar_arrive(&empty[bi % p.NSV]);
-            } else if (!desc) {
-                mbar_arrive(&empty[bi % p.NSH]);
-                if (last) for (int qq = bi + 1; qq < p.NQ; ++qq) mbar_arrive(&empty[qq % p.NSH]);
-            } else {
-                if (bi + 1 < p.NQ) mbar_arrive(&empty[(bi + 1) % p.NSH]);
-                if (last) mbar_arrive(&empty[bi % p.NSH]);
-            }
-        }
     };
     auto block_setup = [&](int bi) -> uint32_t {        // returns the block's chunk-slot offset (horizontal)
         if constexpr (!VH) {
@@ -208,193 +221,112 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
         }
     };
 
-    // ================= pass 1: scan order, checkpoints =================================================
-    float h[P];
+    // ================= pass 1: scan order, checkpoints (ROLE_A; ROLE_F only follows the ring) ===========
+    rs.begin_pass(REV);
+    {
+        float h[P];
 #pragma unroll
-    for (int e = 0; e < P; ++e) {
-        h[e] = 0.f;
-        if (p.h0 && ok[e]) h[e] = ld_f(reinterpret_cast<const ST*>(p.h0) + pc * Lmax + P * lane + e);
-    }
-    begin_pass(REV);
-    for (int n = 0; n < NB; ++n) {
-        const int bi = REV ? NB - 1 - n : n;
-        const int nb = min(kBlk, Ls - kBlk * bi);
-        acquire(bi, REV);
-#pragma unroll
-        for (int e = 0; e < P; ++e) sts32(cks + (bi * P + e) * 128, h[e]);
-        const uint32_t so = block_setup(bi);
-#pragma unroll
-        for (int t = 0; t < kBlk; ++t) {
-            const int tl = REV ? kBlk - 1 - t : t;
-            if (tl < nb) {
-                float hn[P];
-                fwd_step(h, tl, so, hn);
-#pragma unroll
-                for (int e = 0; e < P; ++e) h[e] = hn[e];
-            }
+        for (int e = 0; e < P; ++e) {
+            h[e] = 0.f;
+            if (ROLE == ROLE_A && p.h0 && ok[e]) h[e] = ld_f(reinterpret_cast<const ST*>(p.h0) + pc * Lmax + P * lane + e);
         }
-        release(bi, REV, n == NB - 1);
+        for (int n = 0; n < NB; ++n) {
+            const int bi = REV ? NB - 1 - n : n;
+            const int nb = min(kBlk, Ls - kBlk * bi);
+            rs.acquire(bi, REV);
+            if constexpr (ROLE == ROLE_A) {
+#pragma unroll
+                for (int e = 0; e < P; ++e) sts32(cks + (bi * P + e) * 128, h[e]);
+                const uint32_t so = block_setup(bi);
+#pragma unroll
+                for (int t = 0; t < kBlk; ++t) {
+                    const int tl = REV ? kBlk - 1 - t : t;
+                    if (tl < nb) {
+                        float hn[P];
+                        fwd_step(h, tl, so, hn);
+#pragma unroll
+                        for (int e = 0; e < P; ++e) h[e] = hn[e];
+                    }
+                }
+            }
+            rs.release(bi, REV, n == NB - 1);
+        }
     }
+    // the checkpoints written by ROLE_A are read by ROLE_F of the same channel
+    asm volatile("bar.sync %0, 64;" ::"r"(2 + c) : "memory");
 
     // ================= pass 2: reverse order ===========================================================
     constexpr bool desc2 = !REV;
     float carry[P];
 #pragma unroll
     for (int e = 0; e < P; ++e) carry[e] = 0.f;
-    begin_pass(desc2);
+    rs.begin_pass(desc2);
     for (int n = 0; n < NB; ++n) {
         const int bi = desc2 ? NB - 1 - n : n;
         const int nb = min(kBlk, Ls - kBlk * bi);
-        acquire(bi, desc2);
+        rs.acquire(bi, desc2);
         const uint32_t so = block_setup(bi);
-        float hs[kBlk + 1][P];                  // hs[t] = state entering the t-th step (scan order) of the block
+        bs.producer_wait();
+        if constexpr (ROLE == ROLE_F) {
+            // hs[t] = state entering the t-th step (scan order) of the block
+            const uint32_t hw = hbuf + bs.buf() * ((kBlk + 1) * P * 128);
+            float hs[kBlk + 1][P];
 #pragma unroll
-        for (int e = 0; e < P; ++e) hs[0][e] = lds32(cks + (bi * P + e) * 128);
+            for (int e = 0; e < P; ++e) { hs[0][e] = lds32(cks + (bi * P + e) * 128); sts32(hw + e * 128, hs[0][e]); }
 #pragma unroll
-        for (int t = 0; t < kBlk; ++t) {
-            const int tl = REV ? kBlk - 1 - t : t;
-            if (tl < nb) {
-                fwd_step(hs[t], tl, so, hs[t + 1]);
-            } else {
-#pragma unroll
-                for (int e = 0; e < P; ++e) hs[t + 1][e] = hs[t][e];
-            }
-        }
-        // per-block output / accumulator addresses
-        const int l0 = kBlk * bi;                                   // first image line of the block
-        uint32_t dxv = 0, thb = 0;
-        ST *du_b = nullptr, *dl_b = nullptr;
-        if constexpr (!VH) {
-            dxv = dxs + ((uint32_t)l0 * p.Wp + P * lane) * 4;
-            du_b = du_l + (size_t)l0 * W;
-            dl_b = dl_l + (size_t)l0 * W;
-        } else {
-            thb = (uint32_t)((bi & 1) * kBlk) * ES;
-        }
-#pragma unroll
-        for (int tt = 0; tt < kBlk; ++tt) {
-            const int t = kBlk - 1 - tt;
-            const int tl = REV ? kBlk - 1 - t : t;
-            if (tl < nb) {
-                raw_t w0r[P], w1r[P], w2r[P], lr[P], xr[P], ur[P], dyr[P];
-#pragma unroll
-                for (int e = 0; e < P; ++e) {
-                    ur[e] = ldr(KU, tl, so, e); dyr[e] = ldr(KDY, tl, so, e);
-                    lr[e] = ldr(KLAM, tl, so, e); xr[e] = ldr(KX, tl, so, e);
-                    w0r[e] = ldr(KW0, tl, so, e); w1r[e] = ldr(KW1, tl, so, e); w2r[e] = ldr(KW2, tl, so, e);
-                }
-                float gh[P];
-#pragma unroll
-                for (int e = 0; e < P; ++e) gh[e] = maskf(E::fma2(dyr[e], ur[e], carry[e]), okm[e]);
-                // du, dlambda
-#pragma unroll
-                for (int e = 0; e < P; ++e) {
-                    const raw_t duv = E::pack(E::f(dyr[e]) * hs[t + 1][e]);
-                    const raw_t dlv = E::pack(E::f(xr[e]) * gh[e]);
-                    if constexpr (!VH) {
-                        if (w_du && ok[e]) E::stg(du_b + tl * W + e, duv);
-                        if (w_dl && ok[e]) E::stg(dl_b + tl * W + e, dlv);
-                    } else {
-                        if (w_du && ok[e]) E::sts(tlh[e] + thb + tl * ES, duv);
-                        if (w_dl && ok[e]) E::sts(tlh[e] + tplane + thb + tl * ES, dlv);
-                    }
-                }
-                // dx += lambda * gh
-                if (w_dx) {
-#pragma unroll
-                    for (int e = 0; e < P; ++e) {
-                        const uint32_t a = VH ? dxh[e] + (l0 + tl) * 4 : dxv + (tl * p.Wp + e) * 4;
-                        if (ok[e]) sts32(a, fmaf(E::f(lr[e]), gh[e], lds32(a)));
-                    }
-                }
-                // dw3 partials of this channel: gh * h[s-1, p+k-1]
-                if (w_dw) {
-                    const float hpl = maskf(__shfl_up_sync(FULLM, hs[t][P - 1], 1), m_first);
-                    const float hpr = maskf(__shfl_down_sync(FULLM, hs[t][0], 1), m_31);
-#pragma unroll
-                    for (int e = 0; e < P; ++e) {
-                        const float left = e ? hs[t][e - 1] : hpl;
-                        const float right = e < P - 1 ? hs[t][e + 1] : hpr;
-                        const uint32_t a = exw + (tl * P + e) * 128;
-                        sts32(a, gh[e] * left);
-                        sts32(a + kBlk * P * 128, gh[e] * hs[t][e]);
-                        sts32(a + 2 * kBlk * P * 128, gh[e] * right);
-                    }
-                }
-                // carry = w[s]^T gh: position p receives from p-1 (its tap k=2), p (k=1), p+1 (k=0)
-                float a2[P], c0[P];
-#pragma unroll
-                for (int e = 0; e < P; ++e) {
-                    const float w0f = e == 0 ? maskf(E::f(w0r[e]), m_first) : E::f(w0r[e]);
-                    a2[e] = maskf(E::f(w2r[e]), m_w2[e]) * gh[e];
-                    c0[e] = w0f * gh[e];
-                }
-                const float al = maskf(__shfl_up_sync(FULLM, a2[P - 1], 1), m_first);
-                const float cr = maskf(__shfl_down_sync(FULLM, c0[0], 1), m_31);
-#pragma unroll
-                for (int e = 0; e < P; ++e) {
-                    float acc = fmaf(E::f(w1r[e]), gh[e], e ? a2[e - 1] : al);
-                    acc += e < P - 1 ? c0[e + 1] : cr;
-                    carry[e] = acc;
-                }
-            }
-        }
-        // dw3 of the block: sum over the group's channels in ascending order, one RNE
-        if (w_dw) {
-            if (NS > 1) chain_bar(NS * 32); else __syncwarp();
-            for (int kt = c; kt < 3 * kBlk; kt += NS) {
-                const int k = kt / kBlk, tl = kt % kBlk;
+            for (int t = 0; t < kBlk; ++t) {
+                const int tl = REV ? kBlk - 1 - t : t;
                 if (tl < nb) {
+                    fwd_step(hs[t], tl, so, hs[t + 1]);
+                } else {
+#pragma unroll
+                    for (int e = 0; e < P; ++e) hs[t + 1][e] = hs[t][e];
+                }
+#pragma unroll
+                for (int e = 0; e < P; ++e) sts32(hw + ((t + 1) * P + e) * 128, hs[t + 1][e]);
+            }
+        } else {
+            const uint32_t gw = gbuf + bs.buf() * (kBlk * P * 128);
+#pragma unroll
+            for (int tt = 0; tt < kBlk; ++tt) {
+                const int t = kBlk - 1 - tt;
+                const int tl = REV ? kBlk - 1 - t : t;
+                if (tl < nb) {
+                    raw_t w0r[P], w1r[P], w2r[P], ur[P], dyr[P];
 #pragma unroll
                     for (int e = 0; e < P; ++e) {
-                        const uint32_t a = exs + ((k * kBlk + tl) * P + e) * 128;
-                        float sum = lds32(a);
-                        for (int s = 1; s < NS; ++s) sum += lds32(a + s * (3 * kBlk * P * 128));
-                        if constexpr (!VH) {
-                            if (ok[e]) E::stg(dw_l + (size_t)k * HW + (size_t)(l0 + tl) * W + e, E::pack(sum));
-                        } else {
-                            const int row = P * lane + e;
-                            if (ok[e]) E::sts(dwtile + ((k * Lp + row) * kTilePitch) * ES + thb + tl * ES, E::pack(sum));
-                        }
+                        ur[e] = ldr(KU, tl, so, e); dyr[e] = ldr(KDY, tl, so, e);
+                        w0r[e] = ldr(KW0, tl, so, e); w1r[e] = ldr(KW1, tl, so, e); w2r[e] = ldr(KW2, tl, so, e);
+                    }
+                    float gh[P];
+#pragma unroll
+                    for (int e = 0; e < P; ++e) {
+                        gh[e] = maskf(E::fma2(dyr[e], ur[e], carry[e]), okm[e]);
+                        sts32(gw + (t * P + e) * 128, gh[e]);
+                    }
+                    // carry = w[s]^T gh: position p receives from p-1 (its tap k=2), p (k=1), p+1 (k=0)
+                    float a2[P], c0[P];
+#pragma unroll
+                    for (int e = 0; e < P; ++e) {
+                        const float w0f = e == 0 ? maskf(E::f(w0r[e]), m_first) : E::f(w0r[e]);
+                        a2[e] = maskf(E::f(w2r[e]), m_w2[e]) * gh[e];
+                        c0[e] = w0f * gh[e];
+                    }
+                    const float al = maskf(__shfl_up_sync(FULLM, a2[P - 1], 1), m_first);
+                    const float cr = maskf(__shfl_down_sync(FULLM, c0[0], 1), m_31);
+#pragma unroll
+                    for (int e = 0; e < P; ++e) {
+                        float acc = fmaf(E::f(w1r[e]), gh[e], e ? a2[e - 1] : al);
+                        acc += e < P - 1 ? c0[e + 1] : cr;
+                        carry[e] = acc;
                     }
                 }
             }
-            if (NS > 1) chain_bar(NS * 32); else __syncwarp();
         }
-        // horizontal outputs: a pair of blocks = 8 columns is complete -> 16-byte row pieces to global
-        if constexpr (VH) {
-            const bool pair_done = desc2 ? ((bi & 1) == 0) : ((bi & 1) == 1 || bi == NB - 1);
-            if (pair_done) {
-                const int col0 = 2 * kBlk * (bi >> 1);
-                const int ncols = min(2 * kBlk, W - col0);
-                const int col = lane & 7, rsub = lane >> 3;
-                __syncwarp();
-                if (col < ncols) {
-                    uint32_t ta = tile + (rsub * kTilePitch + col) * ES;
-                    const size_t o = (size_t)rsub * W + col0 + col;
-                    ST* g0 = du_l + o;
-                    ST* g1 = dl_l + o;
-                    for (int r = rsub; r < Lp; r += 4) {
-                        if (w_du) E::stg(g0, E::lds(ta));
-                        if (w_dl) E::stg(g1, E::lds(ta + tplane));
-                        ta += 4 * kTilePitch * ES; g0 += 4 * W; g1 += 4 * W;
-                    }
-                    if (w_dw)
-                        for (int k = c; k < 3; k += NS) {
-                            uint32_t tw = dwtile + ((k * Lp + rsub) * kTilePitch + col) * ES;
-                            ST* g2 = dw_l + (size_t)k * HW + o;
-                            for (int r = rsub; r < Lp; r += 4) {
-                                E::stg(g2, E::lds(tw));
-                                tw += 4 * kTilePitch * ES; g2 += 4 * W;
-                            }
-                        }
-                }
-                __syncwarp();
-            }
-        }
-        release(bi, desc2, n == NB - 1);
+        bs.producer_done(lane);
+        rs.release(bi, desc2, n == NB - 1);
     }
-    if (p.dh0) {
+    if (ROLE == ROLE_A && p.dh0) {
         ST* d0 = reinterpret_cast<ST*>(p.dh0) + pc * Lmax;
 #pragma unroll
         for (int e = 0; e < P; ++e) {
@@ -402,11 +334,208 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
             if (pos < Lmax) E::stg(d0 + pos, E::pack(ok[e] ? carry[e] : 0.f));
         }
     }
+    // ROLE_A must not overwrite the checkpoints (next direction) while ROLE_F still reads them
+    asm volatile("bar.sync %0, 64;" ::"r"(2 + c) : "memory");
+    pf = rs.pf;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Output warp j of one direction: every block, scan-order step j of ALL channels of the group.  Given
+// h[s], h[s-1] (from the ROLE_F warps) and gh[s] (from the ROLE_A warps) every output is pointwise:
+//     du = dy*h[s]   dlambda = x*gh   dx += lambda*gh   dw3[k] = sum_c gh_c * h_c[s-1, p+k-1]
+// so the sum over the group's channels (Eq. 5: shared taps) is a register
+// accumulation in ascending channel order -- no exchange between warps, no atomics.  A step owns one
+// image line (row or column), so the fp32 dx planes have a single writer per element.
+template <typename ST, int P, bool VH>
+__device__ __forceinline__ void chain_bwd_out(const ChainBwdParams& p, uint8_t* smem, const int d, const int b,
+                                              const int g, const int j, const int lane, uint32_t& pf,
+                                              BlockSync& bs) {
+    using E = Elem<ST>;
+    using raw_t = typename E::raw_t;
+    constexpr int ES = sizeof(ST);
+    constexpr int CB = kBlk * ES;
+    const Shape sh = p.sh;
+    const int H = sh.H, W = sh.W, NS = p.NS;
+    const bool rev = d & 1;
+    const int Ls = VH ? W : H, Lp = VH ? H : W;
+    const int NB = (Ls + kBlk - 1) / kBlk;
+    const uint32_t rowB = (uint32_t)W * ES;
+    const int qd = p.q[d];
+    const size_t HW = (size_t)H * W;
+    const ChPlane* tb = reinterpret_cast<const ChPlane*>(smem + p.off_tab) + d * kChMaxPlanes;
+    const uint32_t ring = smem_u32(smem + p.off_ring);
+    const uint8_t* const sbase = smem - smem_u32(smem);
+    RingSync<VH> rs{reinterpret_cast<uint64_t*>(smem), reinterpret_cast<uint64_t*>(smem) + kChSlots,
+                    p.NSV, p.NSH, p.NQ, lane, 0, pf};
+
+    bool ok[P];
+#pragma unroll
+    for (int e = 0; e < P; ++e) ok[e] = P * lane + e < Lp;
+    const uint32_t m_first = lane == 0 ? 0u : 0xffffffffu;
+    const uint32_t m_31 = lane == 31 ? 0u : 0xffffffffu;
+
+    const size_t pc0 = ((size_t)qd * sh.B + b) * sh.C + (size_t)g * NS;       // plane of channel 0 in [D,B,C]
+    const size_t pw = (((size_t)qd * sh.B + b) * sh.G + g) * 3;                // first tap plane in [D,B,G,3]
+    const bool w_du = p.du != nullptr, w_dl = p.dlam != nullptr, w_dw = p.dw3 != nullptr, w_dx = p.dx != nullptr;
+    ST* du0 = reinterpret_cast<ST*>(p.du) + pc0 * HW;
+    ST* dl0 = reinterpret_cast<ST*>(p.dlam) + pc0 * HW;
+    ST* dw0 = reinterpret_cast<ST*>(p.dw3) + pw * HW;
+    const uint32_t dxs = smem_u32(smem + p.off_dx);                            // [NS][H][Wp] fp32
+    const uint32_t hb0 = smem_u32(smem + p.off_hb) + lane * 4;                 // [NS][2][kBlk+1][P][32]
+    const uint32_t gb0 = smem_u32(smem + p.off_gb) + lane * 4;                 // [NS][2][kBlk][P][32]
+    const uint32_t tile = smem_u32(smem + p.off_tile);                         // [2NS+3][Lp][kTilePitch]
+    const uint32_t tplane = (uint32_t)Lp * kTilePitch * ES;
+
+    uint32_t rowadr[P], rowph[P], rowdx[P], rowtl[P];      // horizontal: per row of this lane
+    if constexpr (VH) {
+#pragma unroll
+        for (int e = 0; e < P; ++e) {
+            const int row = min(P * lane + e, H - 1);
+            rowadr[e] = ring + row * p.hrow;
+            rowph[e] = (uint32_t)(((unsigned long long)row * rowB) % CB);
+            rowdx[e] = (uint32_t)row * p.Wp * 4;
+            rowtl[e] = (uint32_t)row * kTilePitch * ES;
+        }
+    }
+
+    // pass 1: nothing to do, follow the ring
+    rs.begin_pass(rev);
+    for (int n = 0; n < NB; ++n) {
+        const int bi = rev ? NB - 1 - n : n;
+        rs.acquire(bi, rev);
+        rs.release(bi, rev, n == NB - 1);
+    }
+    const bool desc2 = !rev;
+    rs.begin_pass(desc2);
+    const int t = j;                                     // scan-order step of every block this warp owns
+    const int tl = rev ? kBlk - 1 - t : t;               // its image-local line
+    for (int n = 0; n < NB; ++n) {
+        const int bi = desc2 ? NB - 1 - n : n;
+        const int nb = min(kBlk, Ls - kBlk * bi);
+        rs.acquire(bi, desc2);
+        bs.consumer_wait();
+        if (tl < nb) {
+            const int li = kBlk * bi + tl;                                       // image line (row / column)
+            const uint32_t hoff = bs.buf() * ((kBlk + 1) * P * 128) + t * P * 128;
+            const uint32_t goff = bs.buf() * (kBlk * P * 128) + t * P * 128;
+            const uint32_t so = VH ? (uint32_t)(bi % p.NSH) * CB + tl * ES : 0u;
+            const uint32_t vst = VH ? 0u : ring + (bi % p.NSV) * p.vstage + lane * (P * ES) + tl * rowB;
+            const uint32_t rb = ((uint32_t)(kBlk * bi) * rowB) & 15u;
+            const uint32_t cs = (uint32_t)((bi & 1) * kBlk + tl) * ES;
+            float dw[3][P];
+#pragma unroll
+            for (int e = 0; e < P; ++e) { dw[0][e] = 0.f; dw[1][e] = 0.f; dw[2][e] = 0.f; }
+#pragma unroll 1
+            for (int c = 0; c < NS; ++c) {
+                const uint32_t hc = hb0 + (uint32_t)c * 2 * (kBlk + 1) * P * 128 + hoff;
+                const uint32_t gc = gb0 + (uint32_t)c * 2 * kBlk * P * 128 + goff;
+                float hn[P], hp[P], gh[P];
+#pragma unroll
+                for (int e = 0; e < P; ++e) {
+                    hp[e] = lds32(hc + e * 128);
+                    hn[e] = lds32(hc + (P + e) * 128);
+                    gh[e] = lds32(gc + e * 128);
+                }
+                const float hpl = maskf(lds32(hc + (P - 1) * 128 - 4), m_first);     // h[s-1] of position p-1 (lane-1)
+                const float hpr = maskf(lds32(hc + 4), m_31);                        // h[s-1] of position p+1 (lane+1)
+                // operand addresses: lambda, x, dy planes of channel c
+                raw_t lr[P], xr[P], dyr[P];
+                {
+                    const int sl = 3 + c, sx = 3 + NS + c, sy = 3 + 3 * NS + c;
+                    const uint32_t bl = (uint32_t)tb[sl].b0, bx = (uint32_t)tb[sx].b0, by = (uint32_t)tb[sy].b0;
+#pragma unroll
+                    for (int e = 0; e < P; ++e) {
+                        uint32_t al, ax, ay;
+                        if constexpr (!VH) {
+                            al = vst + sl * p.vslot + ((bl + rb) & 15u) + e * ES;
+                            ax = vst + sx * p.vslot + ((bx + rb) & 15u) + e * ES;
+                            ay = vst + sy * p.vslot + ((by + rb) & 15u) + e * ES;
+                        } else {
+                            al = rowadr[e] + sl * p.hplane + ((bl + rowph[e]) & (CB - 1)) + so;
+                            ax = rowadr[e] + sx * p.hplane + ((bx + rowph[e]) & (CB - 1)) + so;
+                            ay = rowadr[e] + sy * p.hplane + ((by + rowph[e]) & (CB - 1)) + so;
+                        }
+                        lr[e] = *reinterpret_cast<const raw_t*>(sbase + al);
+                        xr[e] = *reinterpret_cast<const raw_t*>(sbase + ax);
+                        dyr[e] = *reinterpret_cast<const raw_t*>(sbase + ay);
+                    }
+                }
+#pragma unroll
+                for (int e = 0; e < P; ++e) {
+                    const float left = e ? hp[e - 1] : hpl;
+                    const float right = e < P - 1 ? hp[e + 1] : hpr;
+                    dw[0][e] = fmaf(gh[e], left, dw[0][e]);
+                    dw[1][e] = fmaf(gh[e], hp[e], dw[1][e]);
+                    dw[2][e] = fmaf(gh[e], right, dw[2][e]);
+                    const raw_t duv = E::pack(E::f(dyr[e]) * hn[e]);
+                    const raw_t dlv = E::pack(E::f(xr[e]) * gh[e]);
+                    if constexpr (!VH) {
+                        const size_t o = (size_t)c * HW + (size_t)li * W + P * lane + e;
+                        if (w_du && ok[e]) E::stg(du0 + o, duv);
+                        if (w_dl && ok[e]) E::stg(dl0 + o, dlv);
+                        if (w_dx && ok[e]) {
+                            const uint32_t a = dxs + (((uint32_t)c * H + li) * p.Wp + P * lane + e) * 4;
+                            sts32(a, fmaf(E::f(lr[e]), gh[e], lds32(a)));
+                        }
+                    } else {
+                        if (w_du && ok[e]) E::sts(tile + c * tplane + rowtl[e] + cs, duv);
+                        if (w_dl && ok[e]) E::sts(tile + (NS + c) * tplane + rowtl[e] + cs, dlv);
+                        if (w_dx && ok[e]) {
+                            const uint32_t a = dxs + (uint32_t)c * H * p.Wp * 4 + rowdx[e] + li * 4;
+                            sts32(a, fmaf(E::f(lr[e]), gh[e], lds32(a)));
+                        }
+                    }
+                }
+            }
+            if (w_dw) {
+#pragma unroll
+                for (int k = 0; k < 3; ++k)
+#pragma unroll
+                    for (int e = 0; e < P; ++e) {
+                        if constexpr (!VH) {
+                            if (ok[e]) E::stg(dw0 + (size_t)k * HW + (size_t)li * W + P * lane + e, E::pack(dw[k][e]));
+                        } else {
+                            if (ok[e]) E::sts(tile + (2 * NS + k) * tplane + rowtl[e] + cs, E::pack(dw[k][e]));
+                        }
+                    }
+            }
+        }
+        bs.consumer_done(lane);
+        // horizontal outputs: a pair of blocks = 8 columns is complete -> 16-byte row pieces to global
+        if constexpr (VH) {
+            const bool pair_done = desc2 ? ((bi & 1) == 0) : ((bi & 1) == 1 || bi == NB - 1);
+            if (pair_done) {
+                asm volatile("bar.sync 10, 128;" ::: "memory");
+                const int col0 = 2 * kBlk * (bi >> 1);
+                const int ncols = min(2 * kBlk, W - col0);
+                const int col = lane & 7, rsub = lane >> 3;
+                if (col < ncols) {
+                    for (int pl = j; pl < 2 * NS + 3; pl += kBlk) {
+                        ST* gp;
+                        if (pl < NS) gp = w_du ? du0 + (size_t)pl * HW : nullptr;
+                        else if (pl < 2 * NS) gp = w_dl ? dl0 + (size_t)(pl - NS) * HW : nullptr;
+                        else gp = w_dw ? dw0 + (size_t)(pl - 2 * NS) * HW : nullptr;
+                        if (gp) {
+                            gp += (size_t)rsub * W + col0 + col;
+                            uint32_t ta = tile + pl * tplane + (rsub * kTilePitch + col) * ES;
+                            for (int r = rsub; r < Lp; r += 4) {
+                                E::stg(gp, E::lds(ta));
+                                ta += 4 * kTilePitch * ES; gp += 4 * W;
+                            }
+                        }
+                    }
+                }
+                asm volatile("bar.sync 10, 128;" ::: "memory");
+            }
+        }
+        rs.release(bi, desc2, n == NB - 1);
+    }
+    pf = rs.pf;
 }
 
 // ---------------------------------------------------------------------------------------------------
 template <typename ST, int P>
-__global__ void __launch_bounds__(32 * (kChNPW + kChMaxNS), 1)
+__global__ void __launch_bounds__(32 * (kChNPW + 2 * kChMaxNS + kChNO), 1)
 chain_bwd_kernel(const ChainBwdParams p) {
     constexpr int ES = sizeof(ST);
     constexpr int CB = kBlk * ES;
@@ -448,7 +577,8 @@ chain_bwd_kernel(const ChainBwdParams p) {
         }
     }
     if (threadIdx.x == 0) {
-        for (int s = 0; s < kChSlots; ++s) { mbar_init(&full[s], kChNPW * 33); mbar_init(&empty[s], NS); }
+        for (int s = 0; s < kChSlots; ++s) { mbar_init(&full[s], kChNPW * 33); mbar_init(&empty[s], 2 * NS + kChNO); }
+        for (int s = 0; s < 2; ++s) { mbar_init(&empty[kChSlots + s], 2 * NS); mbar_init(&empty[kChSlots + 2 + s], kChNO); }
         mbar_init_fence();
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // zeros (generic proxy) before bulk copies
@@ -551,14 +681,33 @@ chain_bwd_kernel(const ChainBwdParams p) {
                 }
             }
         }
-    } else if (warp < kChNPW + NS) {
-        // ---------------- chain warp of channel c ------------------------------------------------------
-        const int c = warp - kChNPW;
+    } else if (warp < kChNPW + 2 * NS) {
+        // ---------------- chain warps: ROLE_A (pass 1 + adjoint chain) and ROLE_F (recompute) of channel c --
+        const bool roleF = warp >= kChNPW + NS;
+        const int c = warp - kChNPW - (roleF ? NS : 0);
         uint32_t pf = 0;
-        if (p.q[0] >= 0) chain_bwd_dir<ST, P, false, false>(p, smem, 0, b, g, c, lane, pf);
-        if (p.q[1] >= 0) chain_bwd_dir<ST, P, false, true>(p, smem, 1, b, g, c, lane, pf);
-        if (p.q[2] >= 0) chain_bwd_dir<ST, P, true, false>(p, smem, 2, b, g, c, lane, pf);
-        if (p.q[3] >= 0) chain_bwd_dir<ST, P, true, true>(p, smem, 3, b, g, c, lane, pf);
+        BlockSync bs{empty + kChSlots, empty + kChSlots + 2, 0u};
+        if (!roleF) {
+            if (p.q[0] >= 0) chain_bwd_dir<ST, P, false, false, ROLE_A>(p, smem, 0, b, g, c, lane, pf, bs);
+            if (p.q[1] >= 0) chain_bwd_dir<ST, P, false, true, ROLE_A>(p, smem, 1, b, g, c, lane, pf, bs);
+            if (p.q[2] >= 0) chain_bwd_dir<ST, P, true, false, ROLE_A>(p, smem, 2, b, g, c, lane, pf, bs);
+            if (p.q[3] >= 0) chain_bwd_dir<ST, P, true, true, ROLE_A>(p, smem, 3, b, g, c, lane, pf, bs);
+        } else {
+            if (p.q[0] >= 0) chain_bwd_dir<ST, P, false, false, ROLE_F>(p, smem, 0, b, g, c, lane, pf, bs);
+            if (p.q[1] >= 0) chain_bwd_dir<ST, P, false, true, ROLE_F>(p, smem, 1, b, g, c, lane, pf, bs);
+            if (p.q[2] >= 0) chain_bwd_dir<ST, P, true, false, ROLE_F>(p, smem, 2, b, g, c, lane, pf, bs);
+            if (p.q[3] >= 0) chain_bwd_dir<ST, P, true, true, ROLE_F>(p, smem, 3, b, g, c, lane, pf, bs);
+        }
+    } else if (warp < kChNPW + 2 * NS + kChNO) {
+        // ---------------- output warp j: step j of every block, all channels -----------------------------
+        const int j = warp - kChNPW - 2 * NS;
+        uint32_t pf = 0;
+        BlockSync bs{empty + kChSlots, empty + kChSlots + 2, 0u};
+        for (int d = 0; d < 4; ++d) {
+            if (p.q[d] < 0) continue;
+            if (d < 2) chain_bwd_out<ST, P, false>(p, smem, d, b, g, j, lane, pf, bs);
+            else       chain_bwd_out<ST, P, true>(p, smem, d, b, g, j, lane, pf, bs);
+        }
     }
     __syncthreads();
 
@@ -573,12 +722,12 @@ chain_bwd_kernel(const ChainBwdParams p) {
 }
 
 // ---- host side -----------------------------------------------------------------------------------
-static size_t chain_bwd_layout(const Shape& sh, int es, int P, int NSV, int NSH, bool want_dw, ChainBwdParams* prm) {
+static size_t chain_bwd_layout(const Shape& sh, int es, int P, int NSV, int NSH, ChainBwdParams* prm) {
     const int NS = sh.cg(), np = 3 + 4 * NS;
     const bool vact = sh.mask & 3u, hact = sh.mask & 12u;
     const int CB = kBlk * es;
     const int Lmax = sh.Lmax();
-    size_t off = 2 * kChSlots * sizeof(uint64_t);
+    size_t off = kChBars * sizeof(uint64_t);
     prm->off_tab = (uint32_t)off;
     off += (size_t)4 * kChMaxPlanes * sizeof(ChPlane);
     off = (off + 127) / 128 * 128;
@@ -601,14 +750,13 @@ static size_t chain_bwd_layout(const Shape& sh, int es, int P, int NSV, int NSH,
     prm->ckpt_warp = (uint32_t)((size_t)NBmax * P * 32 * 4);
     prm->off_ckpt = (uint32_t)off;
     off += (size_t)NS * prm->ckpt_warp;
-    prm->off_exch = (uint32_t)off;
-    if (want_dw) off += (size_t)NS * 3 * kBlk * P * 32 * 4;
-    off = (off + 127) / 128 * 128;
-    prm->tile_warp = (uint32_t)(((size_t)2 * sh.H * kTilePitch * es + 15) / 16 * 16);
+    off += 128;                                                  // the output warps read one float before / after a line
+    prm->off_hb = (uint32_t)off;
+    off += (size_t)NS * 2 * (kBlk + 1) * P * 32 * 4;
+    prm->off_gb = (uint32_t)off;
+    off += (size_t)NS * 2 * kBlk * P * 32 * 4 + 128;
     prm->off_tile = (uint32_t)off;
-    if (hact) off += (size_t)NS * prm->tile_warp;
-    prm->off_dwtile = (uint32_t)off;
-    if (hact && want_dw) off += ((size_t)3 * sh.H * kTilePitch * es + 15) / 16 * 16;
+    if (hact) off += ((size_t)(2 * NS + 3) * sh.H * kTilePitch * es + 15) / 16 * 16;
     off = (off + 15) / 16 * 16;
     prm->total = (uint32_t)off;
     return off;
@@ -637,7 +785,7 @@ int chain_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li) {
     bool fit = false;
     for (int NSH = 6; NSH >= 3 && !fit; --NSH)
         for (int NSV = 4; NSV >= 2 && !fit; --NSV)
-            if (NSH <= kChSlots && chain_bwd_layout(sh, ES, P, NSV, NSH, a.dw3 != nullptr, &prm) <= (size_t)kMaxSmemOptin) {
+            if (NSH <= kChSlots && chain_bwd_layout(sh, ES, P, NSV, NSH, &prm) <= (size_t)kMaxSmemOptin) {
                 prm.NSV = NSV; prm.NSH = NSH;
                 fit = true;
             }
@@ -656,7 +804,7 @@ int chain_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li) {
     prm.bytes_w = (unsigned long long)sh.D() * sh.B * sh.G * 3 * sh.H * sh.W * ES;
     int q = 0;
     for (int d = 0; d < 4; ++d) prm.q[d] = (sh.mask >> d & 1u) ? q++ : -1;
-    const int threads = 32 * (kChNPW + NS), items = sh.B * sh.G;
+    const int threads = 32 * (kChNPW + 2 * NS + kChNO), items = sh.B * sh.G;
     int rc = GSPN_EUNSUPPORTED;
     switch (P) {
     case 1: rc = launch_chain_bwd<ST, 1>(prm, items, threads, st); break;
