@@ -1,25 +1,28 @@
 // gspn_chain_bwd.cu -- fused backward scan of libgspn, "chain" design:
-// ONE launch, one CTA per (b, group) unit, one WARP per channel of the group.
+// ONE launch, one CTA per (b, group) unit, the serial recurrences on dedicated WARPS (one per channel
+// and role), every pointwise output on separate output warps.
 //
 // The adjoint recurrence (include/gspn.h "Backward scan"; derived from Eq. 1-2,
-// the paper reports backward timings only).  Per direction the
-// warp of channel c makes two passes over the scan line blocks of kBlk = 4 steps:
-//   pass 1 (scan order)    h[s] = w[s] h[s-1] + lambda[s]*x[s], h in registers, the state entering
-//                          each block kept as a checkpoint in shared memory (fp32);
-//   pass 2 (reverse order) per block: h of the block's steps recomputed from its checkpoint into
-//                          registers, then gh[s] = dy[s]*u[s] + carry; du = dy*h[s];
-//                          dlambda = x*gh; dx += lambda*gh; dw3[k] partial = gh * h[s-1, p+k-1];
-//                          carry = w[s]^T gh  (neighbours by warp shuffle, no block barrier).
+// the paper reports backward timings only).  Per direction, over
+// blocks of kBlk = 4 scan steps:
+//   pass 1 (scan order)    ROLE_A warp of channel c: h[s] = w[s] h[s-1] + lambda[s]*x[s], h in
+//                          registers, the state entering each block kept as an fp32 checkpoint on chip;
+//   pass 2 (reverse order) ROLE_F warp of channel c: h of the block's steps recomputed from its
+//                          checkpoint;  ROLE_A warp: gh[s] = dy[s]*u[s] + carry, carry = w[s]^T gh
+//                          (neighbours by warp shuffle, no block barrier);  both hand their 4 lines to
+//                          the output warps through a double-buffered fp32 block buffer (mbarriers);
+//                          output warp j: step j of the block for ALL channels of the group:
+//                          du = dy*h[s], dlambda = x*gh, dx += lambda*gh, dw3[k] = sum_c gh_c*h_c[s-1,p+k-1].
 // dx of the group's channels is accumulated over the directions in an fp32 plane per channel on chip
-// (the directions run one after another, so the plane has a single writer) and rounded once at the
-// end.  dw3 (Eq. 5: taps shared by the channels of a group) is reduced over the
-// channels through a small exchange buffer once per block, in ascending channel order (deterministic,
-// no atomics).  Vertical outputs are stored straight from registers (lanes own consecutive columns);
-// horizontal outputs go through 8-column tiles so that every store instruction writes 16-byte row
-// pieces (the transposed tile on the way out).
+// (directions run one after another and a step owns one image line, so every element has a single
+// writer) and rounded once at the end.  dw3 (Eq. 5: taps shared by the channels of a group,
+// PAPER.md:131-134) is summed over the channels in registers, in ascending channel order
+// (deterministic, no atomics, no exchange between warps).  Vertical outputs are stored straight from
+// registers (lanes own consecutive columns); horizontal outputs go through 8-column tiles so that every
+// store instruction writes 16-byte row pieces (the transposed tile on the way out).
 //
-// Operands: gspn_chain.cuh.  One producer warp streams, for the current direction and pass, a ring of
-// stages: for T->B / B->T a block of 4 image rows of every operand plane (one 1-D bulk copy per plane
+// Operands: gspn_chain.cuh.  kChNPW producer warps stream, for the current direction and pass, a ring
+// of stages: for T->B / B->T a block of 4 image rows of every operand plane (one 1-D bulk copy per plane
 // over its 16-byte-aligned superset), for L->R / R->L one chunk column (4 columns of every row of
 // every plane, cp.async of the aligned chunk; a row keeps NSH+1 chunk slots contiguous, slot NSH
 // mirrors slot 0, so the two chunks a block of 4 columns touches are always contiguous).

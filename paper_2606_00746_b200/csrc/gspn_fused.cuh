@@ -38,12 +38,12 @@ __device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
         "{\n"
         ".reg .pred p;\n"
         "GSPN_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
         "@p bra GSPN_DONE;\n"
         "bra GSPN_WAIT;\n"
         "GSPN_DONE:\n"
         "}\n" ::"r"(smem_u32(b)),
-        "r"(parity)
+        "r"(parity), "r"(0x989680)      // suspend-time hint: a waiting warp sleeps instead of spinning on issue slots
         : "memory");
 }
 

@@ -94,6 +94,36 @@ def test_bwd_direction_masks_and_h0(mask, impl):
         assert r["ok"], (dtype, r)
 
 
+def _chain_or_skip(fn):
+    """Run a check with the chain kernels forced; shapes they do not hold on chip are skipped."""
+    try:
+        return fn()
+    except gspn.GspnError as ex:
+        if ex.status == 2:          # GSPN_EUNSUPPORTED
+            pytest.skip(str(ex))
+        raise
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("shape", BWD_SHAPES + [(1, 8, 73, 73, 2), (1, 2, 128, 128, 2), (1, 2, 100, 36, 1)],
+                         ids=_ids(BWD_SHAPES + [(1, 8, 73, 73, 2), (1, 2, 128, 128, 2), (1, 2, 100, 36, 1)]))
+def test_bwd_chain_small_shapes(shape, dtype):
+    cfg = gi.small_config("bc", *shape, seed=17, backward=True)
+    r = _chain_or_skip(lambda: pu.check_bwd(cfg, dtype, impl=gspn.IMPL_CHAIN))
+    assert r["ok"] and r["variant"] == "chain_bwd", r
+
+
+@pytest.mark.parametrize("mask", [1, 2, 4, 8, 3, 12, 6, 9, 13, 15])
+def test_bwd_chain_direction_masks_and_h0(mask):
+    cfg = gi.small_config("bcm", 2, 4, 9, 12, 2, dir_mask=mask, seed=60 + mask, backward=True)
+    for dtype in ("f32", "bf16"):
+        r = _chain_or_skip(lambda: pu.check_bwd(cfg, dtype, impl=gspn.IMPL_CHAIN, with_h0=True))
+        assert r["ok"], (dtype, r)
+    cfg = gi.small_config("bcm2", 1, 8, 37, 41, 2, dir_mask=mask, seed=80 + mask, backward=True)
+    r = _chain_or_skip(lambda: pu.check_bwd(cfg, "bf16", impl=gspn.IMPL_CHAIN, with_h0=True))
+    assert r["ok"], r
+
+
 def test_bwd_optional_outputs():
     cfg = gi.small_config("opt", 1, 4, 8, 8, 2, seed=3, backward=True)
     t = {k: v.cuda() for k, v in gi.make_inputs(cfg, "f32").items()}
@@ -192,7 +222,7 @@ def test_auto_selects_fused_kernels_where_supported():
     cfg = gi.small_config("sel", 1, 8, 73, 73, 2, seed=9, backward=True)
     r = pu.check_bwd(cfg, "bf16")
     assert r["ok"], r
-    assert r["variant"] == "fused_bwd_group", r["variant"]
+    assert r["variant"] == "chain_bwd", r["variant"]
     assert gspn.gspn_last_launch_count() == 1
     r = pu.check_fwd(cfg, "bf16")
     assert r["ok"] and r["variant"] == "fused_fwd_flat", r
