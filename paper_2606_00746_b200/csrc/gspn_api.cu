@@ -58,8 +58,11 @@ static int fwd_typed(const gspn_args_t* a) {
         rc = naive_fwd_launch<ST>(f, st, &li);
     } else if (a->impl == GSPN_IMPL_FLAT) {
         rc = flat_fwd_launch<ST>(f, st, &li);
+    } else if (a->impl == GSPN_IMPL_CHAIN) {
+        rc = chain_fwd_launch<ST>(f, st, &li);
     } else {
         rc = fused_fwd_launch<ST>(f, st, &li);
+        if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = chain_fwd_launch<ST>(f, st, &li);
         if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = flat_fwd_launch<ST>(f, st, &li);
         if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = naive_fwd_launch<ST>(f, st, &li);
     }

@@ -55,54 +55,6 @@ struct ChainBwdParams {
 
 enum { KW0 = 0, KW1, KW2, KLAM, KX, KU, KDY, KNUM };
 
-__device__ __forceinline__ float maskf(float v, uint32_t m) { return __uint_as_float(__float_as_uint(v) & m); }
-__device__ __forceinline__ float lds32(uint32_t a) {
-    float v;
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
-    return v;
-}
-__device__ __forceinline__ void sts32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v)); }
-
-// ---------------------------------------------------------------------------------------------------
-// Ring hand-shake of a consumer warp.  Block bi (image lines [4bi, 4bi+4)) needs row block bi
-// (vertical) or chunk columns bi and bi+1 (horizontal).  Every consumer warp of the CTA acquires and
-// releases every stage, whether its role has work in it or not, so the mbarrier phases stay aligned.
-template <bool VH>
-struct RingSync {
-    uint64_t *full, *empty;
-    int NSV, NSH, NQ, lane, hq;
-    uint32_t pf;
-    __device__ __forceinline__ void wait_full(int slot) {
-        mbar_wait(&full[slot], (pf >> slot) & 1u);
-        pf ^= 1u << slot;
-    }
-    __device__ __forceinline__ void begin_pass(bool desc) { hq = desc ? NQ - 1 : 0; }
-    __device__ __forceinline__ void acquire(int bi, bool desc) {
-        if constexpr (!VH) {
-            wait_full(bi % NSV);
-        } else if (!desc) {
-            const int need = min(bi + 1, NQ - 1);
-            for (; hq <= need; ++hq) wait_full(hq % NSH);
-        } else {
-            for (; hq >= bi; --hq) wait_full(hq % NSH);
-        }
-    }
-    __device__ __forceinline__ void release(int bi, bool desc, bool last) {
-        __syncwarp();
-        if (lane == 0) {
-            if constexpr (!VH) {
-                mbar_arrive(&empty[bi % NSV]);
-            } else if (!desc) {
-                mbar_arrive(&empty[bi % NSH]);
-                if (last) for (int qq = bi + 1; qq < NQ; ++qq) mbar_arrive(&empty[qq % NSH]);
-            } else {
-                if (bi + 1 < NQ) mbar_arrive(&empty[(bi + 1) % NSH]);
-                if (last) mbar_arrive(&empty[bi % NSH]);
-            }
-        }
-    }
-};
-
 // hand-over of one block's h / gh lines from the chain warps to the output warps (double buffered)
 struct BlockSync {
     uint64_t *ready, *freeb;      // [2] each

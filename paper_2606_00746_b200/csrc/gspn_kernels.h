@@ -23,6 +23,7 @@ template <typename ST> int flat_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st
 // chain kernels (gspn_chain_bwd.cu / gspn_chain_fwd.cu): one warp per scan chain, no block barrier on the
 // serial path, operands staged asynchronously by a producer warp; any H, W <= 128 and storage type.
 template <typename ST> int chain_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
+template <typename ST> int chain_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 
 // merge (gspn_merge.cu)
 template <typename ST>
