@@ -41,18 +41,19 @@ enum { FW0 = 0, FW1, FW2, FLAM, FX, FU, FNUM };
 
 // One direction of one channel.  VH = false: T->B / B->T (lanes own columns), true: L->R / R->L (lanes
 // own rows); REV = the direction walks the image lines downwards.
-template <typename ST, int P, bool VH, bool REV>
+template <typename ST, int P, int CBH, bool VH, bool REV>
 __device__ __forceinline__ void chain_fwd_dir(const ChainFwdParams& p, uint8_t* smem, const int d, const int b,
                                               const int cg0, const int c, const int lane, uint32_t& pf) {
     using E = Elem<ST>;
     using raw_t = typename E::raw_t;
     constexpr int ES = sizeof(ST);
-    constexpr int CB = kBlk * ES;
+    constexpr int CB = CBH;                           // horizontal: bytes of a row per chunk column
+    constexpr int BLK = VH ? CB / ES : kBlk;          // scan steps per block (= ring stage)
     constexpr unsigned FULLM = 0xffffffffu;
     const Shape sh = p.sh;
     const int H = sh.H, W = sh.W, NC = p.NC;
     const int Ls = VH ? W : H, Lp = VH ? H : W, Lmax = sh.Lmax();
-    const int NB = (Ls + kBlk - 1) / kBlk;
+    const int NB = (Ls + BLK - 1) / BLK;
     const uint32_t rowB = (uint32_t)W * ES;
     const int qd = p.q[d];
     const ChPlane* tb = reinterpret_cast<const ChPlane*>(smem + p.off_tab) + d * kCfMaxPlanes;
@@ -104,22 +105,22 @@ __device__ __forceinline__ void chain_fwd_dir(const ChainFwdParams& p, uint8_t* 
     rs.begin_pass(REV);
     for (int n = 0; n < NB; ++n) {
         const int bi = REV ? NB - 1 - n : n;
-        const int nb = min(kBlk, Ls - kBlk * bi);
+        const int nb = min(BLK, Ls - BLK * bi);
         rs.acquire(bi, REV);
         uint32_t so = 0;
         if constexpr (!VH) {
             const uint32_t stage = ring + (bi % p.NSV) * p.vstage;
-            const uint32_t rb = ((uint32_t)(kBlk * bi) * rowB) & 15u;
+            const uint32_t rb = ((uint32_t)(BLK * bi) * rowB) & 15u;
 #pragma unroll
             for (int k = 0; k < FNUM; ++k)
                 vb[k] = stage + sidx[k] * p.vslot + ((phs[k] + rb) & 15u) + lane * (P * ES);
         } else {
             so = (uint32_t)(bi % p.NSH) * CB;
         }
-        const uint32_t yv = ys + ((uint32_t)(kBlk * bi) * p.Wp + P * lane) * 4;      // vertical: (line 4bi, first column)
+        const uint32_t yv = ys + ((uint32_t)(BLK * bi) * p.Wp + P * lane) * 4;      // vertical: (line 4bi, first column)
 #pragma unroll
-        for (int t = 0; t < kBlk; ++t) {
-            const int tl = REV ? kBlk - 1 - t : t;
+        for (int t = 0; t < BLK; ++t) {
+            const int tl = REV ? BLK - 1 - t : t;
             if (tl < nb) {
                 raw_t w0r[P], w1r[P], w2r[P], lr[P], xr[P], ur[P];
 #pragma unroll
@@ -145,7 +146,7 @@ __device__ __forceinline__ void chain_fwd_dir(const ChainFwdParams& p, uint8_t* 
 #pragma unroll
                 for (int e = 0; e < P; ++e) {
                     h[e] = hn[e];
-                    const uint32_t a = VH ? yh[e] + (kBlk * bi + tl) * 4 : yv + (tl * p.Wp + e) * 4;
+                    const uint32_t a = VH ? yh[e] + (BLK * bi + tl) * 4 : yv + (tl * p.Wp + e) * 4;
                     if (ok[e]) sts32(a, fmaf(E::f(ur[e]), hn[e], lds32(a)));
                 }
             }
@@ -156,11 +157,11 @@ __device__ __forceinline__ void chain_fwd_dir(const ChainFwdParams& p, uint8_t* 
 }
 
 // ---------------------------------------------------------------------------------------------------
-template <typename ST, int P>
+template <typename ST, int P, int CBH>
 __global__ void __launch_bounds__(32 * (kCfNPW + kCfMaxNC))
 chain_fwd_kernel(const ChainFwdParams p) {
     constexpr int ES = sizeof(ST);
-    constexpr int CB = kBlk * ES;
+    constexpr int CB = CBH;                           // horizontal chunk columns: CB bytes of every row
     extern __shared__ __align__(1024) uint8_t smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);
     uint64_t* empty = full + kChSlots;
@@ -301,10 +302,10 @@ chain_fwd_kernel(const ChainFwdParams p) {
     } else if (warp < kCfNPW + NC) {
         const int c = warp - kCfNPW;
         uint32_t pf = 0;
-        if (p.q[0] >= 0) chain_fwd_dir<ST, P, false, false>(p, smem, 0, b, c0, c, lane, pf);
-        if (p.q[1] >= 0) chain_fwd_dir<ST, P, false, true>(p, smem, 1, b, c0, c, lane, pf);
-        if (p.q[2] >= 0) chain_fwd_dir<ST, P, true, false>(p, smem, 2, b, c0, c, lane, pf);
-        if (p.q[3] >= 0) chain_fwd_dir<ST, P, true, true>(p, smem, 3, b, c0, c, lane, pf);
+        if (p.q[0] >= 0) chain_fwd_dir<ST, P, CBH, false, false>(p, smem, 0, b, c0, c, lane, pf);
+        if (p.q[1] >= 0) chain_fwd_dir<ST, P, CBH, false, true>(p, smem, 1, b, c0, c, lane, pf);
+        if (p.q[2] >= 0) chain_fwd_dir<ST, P, CBH, true, false>(p, smem, 2, b, c0, c, lane, pf);
+        if (p.q[3] >= 0) chain_fwd_dir<ST, P, CBH, true, true>(p, smem, 3, b, c0, c, lane, pf);
     }
     __syncthreads();
 
@@ -319,10 +320,9 @@ chain_fwd_kernel(const ChainFwdParams p) {
 }
 
 // ---- host side -----------------------------------------------------------------------------------
-static size_t chain_fwd_layout(const Shape& sh, int es, int P, int NC, int NSV, int NSH, ChainFwdParams* prm) {
+static size_t chain_fwd_layout(const Shape& sh, int es, int P, int NC, int NSV, int NSH, int CB, ChainFwdParams* prm) {
     const int np = 3 + 3 * NC;
     const bool vact = sh.mask & 3u, hact = sh.mask & 12u;
-    const int CB = kBlk * es;
     size_t off = 2 * kChSlots * sizeof(uint64_t);
     prm->off_tab = (uint32_t)off;
     off += (size_t)4 * kCfMaxPlanes * sizeof(ChPlane);
@@ -346,9 +346,9 @@ static size_t chain_fwd_layout(const Shape& sh, int es, int P, int NC, int NSV, 
     return off;
 }
 
-template <typename ST, int P>
+template <typename ST, int P, int CBH>
 static int launch_chain_fwd(const ChainFwdParams& prm, int items, int threads, cudaStream_t st) {
-    auto kern = chain_fwd_kernel<ST, P>;
+    auto kern = chain_fwd_kernel<ST, P, CBH>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prm.total);
     if (e != cudaSuccess) { set_error("chain fwd: cudaFuncSetAttribute(%u B): %s", prm.total, cudaGetErrorString(e)); return GSPN_ECUDA; }
     kern<<<items, threads, prm.total, st>>>(prm);
@@ -366,12 +366,17 @@ int chain_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li) {
     if (P > 4) { set_error("chain fwd: max(H,W) = %d > 128", L); return GSPN_EUNSUPPORTED; }
     // channels per CTA: the count (1, 2 or 4, dividing cg) that puts the most chain warps on one SM
     // (228 KB of shared memory per SM, 1 KB reserved per CTA, at most 32 CTAs)
+    // horizontal chunk columns: 16 bytes of every row when rows are not 16-byte aligned (half the copy
+    // requests; the rows' different byte phases spread the row-per-lane reads over the banks), else 8 bytes
+    // (row slots an odd number of 8-byte units apart: 2-way instead of 16-way bank conflicts)
+    const int CBH = ((size_t)sh.W * ES) % 16 ? 16 : (ES == 4 ? 16 : 8);
+    const int NSH = CBH == 16 && ES == 2 ? 3 : 4;
     ChainFwdParams best{};
     int best_warps = 0;
     for (int NC = 1; NC <= kCfMaxNC; NC *= 2) {
         if (cg % NC) continue;
         ChainFwdParams prm{};
-        const size_t need = chain_fwd_layout(sh, ES, P, NC, 4, 4, &prm);
+        const size_t need = chain_fwd_layout(sh, ES, P, NC, 4, NSH, CBH, &prm);
         if (need > (size_t)kMaxSmemOptin) continue;
         int ctas = (int)((size_t)228 * 1024 / (need + 1024));
         if (ctas > 32) ctas = 32;
@@ -385,10 +390,10 @@ int chain_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li) {
         return GSPN_EUNSUPPORTED;
     }
     ChainFwdParams& prm = best;
-    prm.NSV = 4; prm.NSH = 4;
+    prm.NSV = 4; prm.NSH = NSH;
     prm.sh = sh;
     prm.x = a.x; prm.w3 = a.w3; prm.lam = a.lam; prm.u = a.u; prm.h0 = a.h0; prm.y = a.y;
-    prm.NQ = (kBlk * ES - ES + sh.W * ES + kBlk * ES - 1) / (kBlk * ES);
+    prm.NQ = (CBH - ES + sh.W * ES + CBH - 1) / CBH;
     const unsigned long long n = (unsigned long long)sh.B * sh.C * sh.H * sh.W;
     prm.bytes_x = n * ES;
     prm.bytes_c = (unsigned long long)sh.D() * n * ES;
@@ -397,12 +402,14 @@ int chain_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li) {
     for (int d = 0; d < 4; ++d) prm.q[d] = (sh.mask >> d & 1u) ? q++ : -1;
     const int threads = 32 * (kCfNPW + prm.NC), items = sh.B * sh.G * (cg / prm.NC);
     int rc = GSPN_EUNSUPPORTED;
-    switch (P) {
-    case 1: rc = launch_chain_fwd<ST, 1>(prm, items, threads, st); break;
-    case 2: rc = launch_chain_fwd<ST, 2>(prm, items, threads, st); break;
-    case 3: rc = launch_chain_fwd<ST, 3>(prm, items, threads, st); break;
-    case 4: rc = launch_chain_fwd<ST, 4>(prm, items, threads, st); break;
-    }
+    constexpr int CBW = ES == 4 ? 16 : 8;       // the narrow variant (fp32: 16 bytes = 4 columns either way)
+#define GSPN_CF_CASE(PP)                                                                              \
+    case PP:                                                                                          \
+        rc = CBH == CBW ? launch_chain_fwd<ST, PP, CBW>(prm, items, threads, st)                      \
+                        : launch_chain_fwd<ST, PP, 16>(prm, items, threads, st);                      \
+        break;
+    switch (P) { GSPN_CF_CASE(1) GSPN_CF_CASE(2) GSPN_CF_CASE(3) GSPN_CF_CASE(4) }
+#undef GSPN_CF_CASE
     if (rc == GSPN_OK) { li->launches = 1; li->variant = "chain_fwd"; }
     return rc;
 }
