@@ -103,6 +103,7 @@ __device__ __forceinline__ void chain_fwd_dir(const ChainFwdParams& p, uint8_t* 
             h[e] = ld_f(reinterpret_cast<const ST*>(p.h0) + (((size_t)qd * sh.B + b) * sh.C + cg0 + c) * Lmax + P * lane + e);
     }
     rs.begin_pass(REV);
+    uint32_t hso = 0;
     for (int n = 0; n < NB; ++n) {
         const int bi = REV ? NB - 1 - n : n;
         const int nb = min(BLK, Ls - BLK * bi);
@@ -115,7 +116,13 @@ __device__ __forceinline__ void chain_fwd_dir(const ChainFwdParams& p, uint8_t* 
             for (int k = 0; k < FNUM; ++k)
                 vb[k] = stage + sidx[k] * p.vslot + ((phs[k] + rb) & 15u) + lane * (P * ES);
         } else {
-            so = (uint32_t)(bi % p.NSH) * CB;
+            // fold the block's chunk-slot offset into the row addresses once per block
+            const uint32_t nso = (uint32_t)(bi % p.NSH) * CB;
+#pragma unroll
+            for (int e = 0; e < P; ++e)
+#pragma unroll
+                for (int k = 0; k < FNUM; ++k) hb[k][e] += nso - hso;
+            hso = nso;
         }
         const uint32_t yv = ys + ((uint32_t)(BLK * bi) * p.Wp + P * lane) * 4;      // vertical: (line 4bi, first column)
 #pragma unroll
