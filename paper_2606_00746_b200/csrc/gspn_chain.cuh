@@ -65,6 +65,22 @@ template <> __device__ __forceinline__ void cp_async_cb<16>(uint32_t dst, const 
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
 
+// L2 prefetch of [p, p+bytes): p 16-byte aligned, bytes a multiple of 16 (cp.async.bulk.prefetch.L2).  The
+// producers announce the operand planes of a direction before they stream them in small stages, so the
+// stage copies find their lines in L2 instead of paying the DRAM latency once per stage.
+__device__ __forceinline__ void l2_prefetch_bulk(const void* p, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+// prefetch the 16-byte-aligned superset of plane e (HWB bytes long) that lies inside its tensor
+__device__ __forceinline__ void l2_prefetch_plane(const uint8_t* base, unsigned long long b0, unsigned long long tbytes,
+                                                  unsigned long long HWB) {
+    const unsigned long long a0 = b0 & ~15ull;
+    unsigned long long a1 = (b0 + HWB + 15) & ~15ull;
+    const unsigned long long lim = tbytes & ~15ull;
+    if (a1 > lim) a1 = lim;
+    if (a1 > a0) l2_prefetch_bulk(base + a0, (uint32_t)(a1 - a0));
+}
+
 // named barrier among the chain warps of a CTA (the producer warp does not take part)
 __device__ __forceinline__ void chain_bar(int nthreads) {
     asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");

@@ -554,6 +554,10 @@ chain_bwd_kernel(const ChainBwdParams p) {
             if (p.q[d] < 0) continue;
             const bool vh = d >> 1, rev = d & 1;
             const ChPlane* tb = tab + d * kChMaxPlanes;
+            {   // announce every operand plane of this direction to L2
+                const int s = lane * kChNPW + pw;
+                if (s < np) l2_prefetch_plane(tb[s].base, tb[s].b0, tb[s].tbytes, HW * ES);
+            }
             if (vh && !drained) {
                 // row-block stages and chunk columns lay the ring out differently: every slot must be
                 // released before the first chunk column is written
@@ -699,6 +703,9 @@ static size_t chain_bwd_layout(const Shape& sh, int es, int P, int NSV, int NSH,
     size_t ringb = 0;
     if (vact) ringb = (size_t)NSV * prm->vstage;
     if (hact && (size_t)np * prm->hplane + 64 > ringb) ringb = (size_t)np * prm->hplane + 64;
+    // the vertical directions use the whole ring region: as many row-block stages as fit (deeper prefetch)
+    prm->NSV = NSV;
+    if (vact && ringb / prm->vstage > (size_t)NSV) prm->NSV = (int)(ringb / prm->vstage < (size_t)kChSlots ? ringb / prm->vstage : kChSlots);
     off += ringb;
     off = (off + 127) / 128 * 128;
     const int NBmax = (Lmax + kBlk - 1) / kBlk;
@@ -741,7 +748,7 @@ int chain_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li) {
     for (int NSH = 6; NSH >= 3 && !fit; --NSH)
         for (int NSV = 4; NSV >= 2 && !fit; --NSV)
             if (NSH <= kChSlots && chain_bwd_layout(sh, ES, P, NSV, NSH, &prm) <= (size_t)kMaxSmemOptin) {
-                prm.NSV = NSV; prm.NSH = NSH;
+                prm.NSH = NSH;        // prm.NSV was set by the layout
                 fit = true;
             }
     if (!fit) {

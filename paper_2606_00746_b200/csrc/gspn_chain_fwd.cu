@@ -228,6 +228,10 @@ chain_fwd_kernel(const ChainFwdParams p) {
             if (p.q[d] < 0) continue;
             const bool vh = d >> 1, desc = d & 1;
             const ChPlane* tb = tab + d * kCfMaxPlanes;
+            {   // announce every operand plane of this direction to L2
+                const int s = lane * kCfNPW + pw;
+                if (s < np) l2_prefetch_plane(tb[s].base, tb[s].b0, tb[s].tbytes, HW * ES);
+            }
             if (vh && !drained) {
                 // row-block stages and chunk columns lay the ring out differently: every slot must be
                 // released before the first chunk column is written
@@ -347,6 +351,9 @@ static size_t chain_fwd_layout(const Shape& sh, int es, int P, int NC, int NSV, 
     size_t ringb = 0;
     if (vact) ringb = (size_t)NSV * prm->vstage;
     if (hact && (size_t)np * prm->hplane + 64 > ringb) ringb = (size_t)np * prm->hplane + 64;
+    // the vertical directions use the whole ring region: as many row-block stages as fit (deeper prefetch)
+    prm->NSV = NSV;
+    if (vact && ringb / prm->vstage > (size_t)NSV) prm->NSV = (int)(ringb / prm->vstage < (size_t)kChSlots ? ringb / prm->vstage : kChSlots);
     off += ringb;
     off = (off + 15) / 16 * 16;
     prm->total = (uint32_t)off;
@@ -397,7 +404,7 @@ int chain_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li) {
         return GSPN_EUNSUPPORTED;
     }
     ChainFwdParams& prm = best;
-    prm.NSV = 4; prm.NSH = NSH;
+    prm.NSH = NSH;            // prm.NSV was set by the layout
     prm.sh = sh;
     prm.x = a.x; prm.w3 = a.w3; prm.lam = a.lam; prm.u = a.u; prm.h0 = a.h0; prm.y = a.y;
     prm.NQ = (CBH - ES + sh.W * ES + CBH - 1) / CBH;
