@@ -139,7 +139,8 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
         if constexpr (!VH) return *reinterpret_cast<const raw_t*>(sbase + (vb[k] + tl * rowB + e * ES));
         else return *reinterpret_cast<const raw_t*>(sbase + (hb[k][e] + so + tl * ES));
     };
-    auto block_setup = [&](int bi) -> uint32_t {        // returns the block's chunk-slot offset (horizontal)
+    uint32_t hso = 0;
+    auto block_setup = [&](int bi) -> uint32_t {
         if constexpr (!VH) {
             const uint32_t stage = ring + (bi % p.NSV) * p.vstage;
             const uint32_t rb = ((uint32_t)(kBlk * bi) * rowB) & 15u;
@@ -148,7 +149,14 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
                 vb[k] = stage + sidx[k] * p.vslot + ((phs[k] + rb) & 15u) + lane * (P * ES);
             return 0u;
         } else {
-            return (uint32_t)(bi % p.NSH) * CB;
+            // fold the block's chunk-slot offset into the row addresses once per block
+            const uint32_t nso = (uint32_t)(bi % p.NSH) * CB;
+#pragma unroll
+            for (int e = 0; e < P; ++e)
+#pragma unroll
+                for (int k = 0; k < KNUM; ++k) hb[k][e] += nso - hso;
+            hso = nso;
+            return 0u;
         }
     };
 
