@@ -228,3 +228,30 @@ def test_auto_selects_fused_kernels_where_supported():
     assert gspn.gspn_last_launch_count() == 1
     r = pu.check_fwd(cfg, "bf16")
     assert r["ok"] and r["variant"] == "chain_fwd", r
+
+def test_chain_kernels_random_shapes():
+    """Seeded sweep of the chain kernels (forced) over random shapes, masks, dtypes, group sizes and
+    initial states: ragged tails, lines of 1..128 positions, 1/2/4 channels per group."""
+    import random
+    rnd = random.Random(2024)
+    ran = 0
+    for it in range(40):
+        cg = rnd.choice([1, 2, 4]); G = rnd.choice([1, 2, 3]); C = cg * G; B = rnd.choice([1, 2])
+        H = rnd.choice([1, 2, 3, 5, 13, 27, 32, 33, 40, 64, 65, 73, 97, 128])
+        W = rnd.choice([1, 2, 3, 4, 7, 16, 27, 33, 35, 56, 65, 73, 96, 128])
+        if rnd.random() < 0.6:
+            H, W = min(H, 40), min(W, 40)
+        mask = rnd.randint(1, 15); dt = rnd.choice(["f32", "bf16"]); h0 = rnd.random() < 0.4
+        if B * C * H * W <= 8 and dt == "bf16":
+            continue        # the relative-L2 gate is not meaningful for a handful of elements
+        cfg = gi.small_config("rz", B, C, H, W, G, dir_mask=mask, seed=3000 + it, backward=True)
+        for check in (pu.check_fwd, pu.check_bwd):
+            try:
+                r = check(cfg, dt, impl=gspn.IMPL_CHAIN, with_h0=h0)
+            except gspn.GspnError as ex:
+                if ex.status == 2:
+                    continue
+                raise
+            ran += 1
+            assert r["ok"], (check.__name__, (B, C, H, W, G), mask, dt, h0, r)
+    assert ran >= 40
