@@ -85,10 +85,15 @@ static int bwd_typed(const gspn_args_t* a) {
         rc = naive_bwd_launch<ST>(f, st, &li);
     } else if (a->impl == GSPN_IMPL_FUSED) {
         rc = fused_bwd_launch<ST>(f, st, &li);
-    } else {
+    } else if (a->impl == GSPN_IMPL_CHAIN) {
         rc = chain_bwd_launch<ST>(f, st, &li);
-        if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = fused_bwd_launch<ST>(f, st, &li);
-        if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = naive_bwd_launch<ST>(f, st, &li);
+    } else {
+        // lines of at most one warp (378-px config: 27x27): the per-block hand-shakes of the chain kernel cost
+        // more than the group kernel's block barriers (measured: cfg3 2.45 ms group, 2.97 ms chain)
+        const bool small = f.sh.Lmax() <= 32;
+        rc = small ? fused_bwd_launch<ST>(f, st, &li) : chain_bwd_launch<ST>(f, st, &li);
+        if (rc == GSPN_EUNSUPPORTED) rc = small ? chain_bwd_launch<ST>(f, st, &li) : fused_bwd_launch<ST>(f, st, &li);
+        if (rc == GSPN_EUNSUPPORTED) rc = naive_bwd_launch<ST>(f, st, &li);
     }
     if (rc == GSPN_OK) { g_launches = li.launches; g_variant = li.variant; }
     return rc;

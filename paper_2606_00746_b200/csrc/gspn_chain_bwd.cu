@@ -498,7 +498,7 @@ __device__ __forceinline__ void chain_bwd_out(const ChainBwdParams& p, uint8_t* 
 
 // ---------------------------------------------------------------------------------------------------
 template <typename ST, int P>
-__global__ void __launch_bounds__(32 * (kChNPW + 2 * kChMaxNS + kChNO), 1)
+__global__ void __launch_bounds__(32 * (kChNPW + 2 * kChMaxNS + kChNO), P == 1 ? 2 : 1)
 chain_bwd_kernel(const ChainBwdParams p) {
     constexpr int ES = sizeof(ST);
     constexpr int CB = kBlk * ES;
