@@ -60,6 +60,8 @@ static int fwd_typed(const gspn_args_t* a) {
         rc = flat_fwd_launch<ST>(f, st, &li);
     } else if (a->impl == GSPN_IMPL_CHAIN) {
         rc = chain_fwd_launch<ST>(f, st, &li);
+    } else if (a->impl == GSPN_IMPL_PAIR) {
+        rc = pair_fwd_launch<ST>(f, st, &li);
     } else {
         rc = fused_fwd_launch<ST>(f, st, &li);
         if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = chain_fwd_launch<ST>(f, st, &li);
@@ -105,7 +107,7 @@ static int check_ex(const gspn_args_t* a) {
         set_error("gspn_args_t.struct_size=%zu, expected %zu", a->struct_size, sizeof(gspn_args_t));
         return GSPN_EINVAL;
     }
-    if (a->impl < GSPN_IMPL_AUTO || a->impl > GSPN_IMPL_CHAIN) {
+    if (a->impl < GSPN_IMPL_AUTO || a->impl > GSPN_IMPL_PAIR) {
         set_error("unknown impl %d", a->impl);
         return GSPN_EINVAL;
     }

@@ -25,6 +25,10 @@ template <typename ST> int flat_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st
 template <typename ST> int chain_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 template <typename ST> int chain_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 
+// pair kernel (gspn_pair_fwd.cu): one warp carries all channels of a CTA for one direction (shared taps, NC*P
+// independent recurrences per lane), the two opposite directions of an axis run at the same time and share Y.
+template <typename ST> int pair_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
+
 // merge (gspn_merge.cu)
 template <typename ST>
 int merge_launch(const ST* y_dirs, const float* m, ST* y, int D, int B, int C, int H, int W,

@@ -16,8 +16,8 @@ pytestmark = pytest.mark.gpu
 
 IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO]
 IMPL_IDS = ["naive", "auto"]
-FWD_IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO, gspn.IMPL_FLAT, gspn.IMPL_CHAIN]
-FWD_IMPL_IDS = ["naive", "auto", "flat", "chain"]
+FWD_IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO, gspn.IMPL_FLAT, gspn.IMPL_CHAIN, gspn.IMPL_PAIR]
+FWD_IMPL_IDS = ["naive", "auto", "flat", "chain", "pair"]
 
 # (B, C, H, W, G): degenerate lines, W in {1,2,3}, H != W, beyond one warp, ragged tails, cg in {1,C}
 SMALL_SHAPES = [
@@ -32,14 +32,24 @@ def _ids(shapes):
     return ["x".join(map(str, s)) for s in shapes]
 
 
+def _fwd_or_skip(impl, fn):
+    """The pair kernel keeps whole fp32 planes on chip: shapes it reports as unsupported are skipped."""
+    try:
+        return fn()
+    except gspn.GspnError as ex:
+        if impl == gspn.IMPL_PAIR and ex.status == 2:          # GSPN_EUNSUPPORTED
+            pytest.skip(str(ex))
+        raise
+
+
 @pytest.mark.parametrize("impl", FWD_IMPLS, ids=FWD_IMPL_IDS)
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
 @pytest.mark.parametrize("shape", SMALL_SHAPES, ids=_ids(SMALL_SHAPES))
 def test_fwd_small_shapes(shape, dtype, impl):
     cfg = gi.small_config("s", *shape, seed=11)
-    if impl == gspn.IMPL_CHAIN and max(shape[2], shape[3]) > 128:
+    if impl in (gspn.IMPL_CHAIN, gspn.IMPL_PAIR) and max(shape[2], shape[3]) > 128:
         pytest.skip("chain kernels hold lines of at most 128 positions")
-    r = pu.check_fwd(cfg, dtype, impl=impl)
+    r = _fwd_or_skip(impl, lambda: pu.check_fwd(cfg, dtype, impl=impl))
     assert r["ok"], r
 
 
@@ -230,7 +240,7 @@ def test_auto_selects_fused_kernels_where_supported():
     assert r["ok"] and r["variant"] == "chain_fwd", r
 
 def test_chain_kernels_random_shapes():
-    """Seeded sweep of the chain kernels (forced) over random shapes, masks, dtypes, group sizes and
+    """Seeded sweep of the chain kernels and the pair forward kernel (forced) over random shapes, masks, dtypes, group sizes and
     initial states: ragged tails, lines of 1..128 positions, 1/2/4 channels per group."""
     import random
     rnd = random.Random(2024)
@@ -245,13 +255,13 @@ def test_chain_kernels_random_shapes():
         if B * C * H * W <= 8 and dt == "bf16":
             continue        # the relative-L2 gate is not meaningful for a handful of elements
         cfg = gi.small_config("rz", B, C, H, W, G, dir_mask=mask, seed=3000 + it, backward=True)
-        for check in (pu.check_fwd, pu.check_bwd):
+        for check, impl in ((pu.check_fwd, gspn.IMPL_CHAIN), (pu.check_bwd, gspn.IMPL_CHAIN), (pu.check_fwd, gspn.IMPL_PAIR)):
             try:
-                r = check(cfg, dt, impl=gspn.IMPL_CHAIN, with_h0=h0)
+                r = check(cfg, dt, impl=impl, with_h0=h0)
             except gspn.GspnError as ex:
                 if ex.status == 2:
                     continue
                 raise
             ran += 1
-            assert r["ok"], (check.__name__, (B, C, H, W, G), mask, dt, h0, r)
-    assert ran >= 40
+            assert r["ok"], (check.__name__, impl, (B, C, H, W, G), mask, dt, h0, r)
+    assert ran >= 60
