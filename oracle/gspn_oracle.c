@@ -16,6 +16,7 @@
  *   backward the exact adjoint of the above (the paper reports backward
  *            timings only; derivation in gspn_oracle_impl.h)
  *   merge    y = sum_d m[d,c] * y_d                          Eq. (9)
+ *   normalize w = sigmoid(wt) / sum_{N(j)} sigmoid(wt)        Eq. (3), PAPER.md:94-97 (and its adjoint)
  *
  * Precision: double ("truth").  A float build of the same loops, with fmaf in
  * one pinned order and -ffp-contract=off, exists as a diagnostic and as the
@@ -32,6 +33,8 @@
  *         adjoint identity <scan(v),dy> = <v,dx>, dense-matrix transpose on
  *         4x4, group-sum identity for dw3.
  *   merge: numpy einsum on random data.
+ *   normalize: rows sum to one, equal logits give 1/|N(j)|, softmax identity on two taps, scipy expit,
+ *         finite differences and the adjoint identity for its backward, the clamp branch.
  * The paper prints no worked numeric example of Eq. (1), so there is no
  * paper-value fixture; every function above is pinned by the mathematics.
  *
@@ -81,6 +84,93 @@ int gspn_oracle_merge_f64(const double *y_dirs, const double *m, double *y,
                            y_dirs[(((size_t)q * B + b) * C + c) * plane + o];
                 y[((size_t)b * C + c) * plane + o] = acc;
             }
+    return 0;
+}
+
+/*
+ * Row-stochastic normalisation of the raw tap logits, Eq. (3), in the order the paper's fused
+ * kernel names ("sigmoid activation, local reduction, clamping, and division"):
+ *     s_k   = 1 / (1 + exp(-wt_k))                       k = 0, 1, 2  (neighbour -1, 0, +1 on the cross axis)
+ *     S     = sum over the taps k whose neighbour lies inside the grid (the set N(j) of Eq. 3)
+ *     w_k   = s_k / max(S, eps)   for k in N(j),   0 for the out-of-grid taps
+ * wt, w3: [D,B,G,3,H,W]; the cross axis is j for the vertical directions (mask bits 0, 1) and i for the
+ * horizontal ones (bits 2, 3).  eps: the paper gives no clamp bound; reading R17 takes 1e-6.
+ */
+static int norm_valid(int dir, int k, int i, int j, int H, int W)
+{
+    const int p = dir < 2 ? j : i, L = dir < 2 ? W : H;      /* cross position and its extent */
+    if (k == 0) return p > 0;
+    if (k == 2) return p < L - 1;
+    return 1;
+}
+
+int gspn_oracle_normalize_f64(const double *wt, double *w3, int B, int G, int H, int W,
+                              unsigned mask, double eps)
+{
+    if (B < 1 || G < 1 || H < 1 || W < 1 || mask < 1 || mask > 15) return 1;
+    const size_t plane = (size_t)H * W;
+    int q = 0;
+    for (int dir = 0; dir < 4; ++dir) {
+        if (!(mask >> dir & 1u)) continue;
+        for (int bg = 0; bg < B * G; ++bg) {
+            const double *a = wt + ((size_t)q * B * G + bg) * 3 * plane;
+            double *o = w3 + ((size_t)q * B * G + bg) * 3 * plane;
+            for (int i = 0; i < H; ++i)
+                for (int j = 0; j < W; ++j) {
+                    double s[3], S = 0.0;
+                    for (int k = 0; k < 3; ++k) {
+                        s[k] = 1.0 / (1.0 + exp(-a[k * plane + (size_t)i * W + j]));
+                        if (norm_valid(dir, k, i, j, H, W)) S += s[k];
+                    }
+                    const double Sc = S > eps ? S : eps;
+                    for (int k = 0; k < 3; ++k)
+                        o[k * plane + (size_t)i * W + j] = norm_valid(dir, k, i, j, H, W) ? s[k] / Sc : 0.0;
+                }
+        }
+        ++q;
+    }
+    return 0;
+}
+
+/*
+ * Adjoint of the above: dwt_k = s_k (1 - s_k) * dL/ds_k with, for k in N(j),
+ *     dL/ds_k = (dw_k - sum_{k' in N(j)} dw_k' w_k') / S     where the clamp is inactive (S > eps)
+ *     dL/ds_k = dw_k / eps                                    where it is active (the denominator is a constant)
+ * and dwt_k = 0 for the out-of-grid taps (they do not reach any output).
+ */
+int gspn_oracle_normalize_bwd_f64(const double *wt, const double *dw3, double *dwt, int B, int G, int H,
+                                  int W, unsigned mask, double eps)
+{
+    if (B < 1 || G < 1 || H < 1 || W < 1 || mask < 1 || mask > 15) return 1;
+    const size_t plane = (size_t)H * W;
+    int q = 0;
+    for (int dir = 0; dir < 4; ++dir) {
+        if (!(mask >> dir & 1u)) continue;
+        for (int bg = 0; bg < B * G; ++bg) {
+            const size_t base = ((size_t)q * B * G + bg) * 3 * plane;
+            for (int i = 0; i < H; ++i)
+                for (int j = 0; j < W; ++j) {
+                    const size_t o = base + (size_t)i * W + j;
+                    double s[3], S = 0.0;
+                    int v[3];
+                    for (int k = 0; k < 3; ++k) {
+                        s[k] = 1.0 / (1.0 + exp(-wt[o + k * plane]));
+                        v[k] = norm_valid(dir, k, i, j, H, W);
+                        if (v[k]) S += s[k];
+                    }
+                    double dot = 0.0;                      /* sum_k' dw_k' w_k' over N(j) */
+                    if (S > eps)
+                        for (int k = 0; k < 3; ++k)
+                            if (v[k]) dot += dw3[o + k * plane] * (s[k] / S);
+                    for (int k = 0; k < 3; ++k) {
+                        double ds = 0.0;
+                        if (v[k]) ds = S > eps ? (dw3[o + k * plane] - dot) / S : dw3[o + k * plane] / eps;
+                        dwt[o + k * plane] = s[k] * (1.0 - s[k]) * ds;
+                    }
+                }
+        }
+        ++q;
+    }
     return 0;
 }
 

@@ -122,6 +122,36 @@ def merge(y_dirs, m=None):
     return y
 
 
+NORM_EPS = 1e-6      # clamp bound of Eq. (3)'s denominator (reading R17; the paper gives none)
+
+
+def normalize(wt, mask: int, eps: float = NORM_EPS):
+    """w3 = Eq. (3) of the logits wt [D,B,G,3,H,W] (fp64): sigmoid, sum over the in-grid taps, clamp, divide."""
+    wt = _prep(wt, np.float64)
+    D, B, G, three, H, W = wt.shape
+    assert three == 3 and D == popcount(mask)
+    w3 = np.empty_like(wt)
+    rc = _load().gspn_oracle_normalize_f64(_ptr(wt), _ptr(w3), B, G, H, W, ctypes.c_uint(mask),
+                                           ctypes.c_double(eps))
+    if rc != 0:
+        raise ValueError("gspn_oracle_normalize: invalid arguments")
+    return w3
+
+
+def normalize_bwd(wt, dw3, mask: int, eps: float = NORM_EPS):
+    """dwt = adjoint of normalize at wt applied to dw3 (fp64)."""
+    wt = _prep(wt, np.float64)
+    dw3 = _prep(dw3, np.float64)
+    D, B, G, three, H, W = wt.shape
+    assert three == 3 and D == popcount(mask) and dw3.shape == wt.shape
+    dwt = np.empty_like(wt)
+    rc = _load().gspn_oracle_normalize_bwd_f64(_ptr(wt), _ptr(dw3), _ptr(dwt), B, G, H, W,
+                                               ctypes.c_uint(mask), ctypes.c_double(eps))
+    if rc != 0:
+        raise ValueError("gspn_oracle_normalize_bwd: invalid arguments")
+    return dwt
+
+
 def fwd_magnitude(x, w3, lam, u, G: int, mask: int, h0=None):
     """A >= |y| elementwise: the same recurrence on |x|, |lambda|, |u|, |w3|, |h0|.
 

@@ -467,3 +467,129 @@ def test_float_build_tracks_double_build():
     y32 = orc.fwd(xs, ws, ls, us, G, 15)
     assert y32.dtype == np.float32
     assert np.all(np.abs(y32 - y64) <= np.maximum(1e-5 * A, 1e-6))
+
+
+# ----------------------------------------------------------------------------- Eq. (3) normalisation
+def _in_grid(d, k, i, j, H, W):
+    """Tap k of pixel (i,j) has its neighbour inside the grid -- written independently of the oracle."""
+    p, L = (j, W) if d < 2 else (i, H)
+    return not ((k == 0 and p == 0) or (k == 2 and p == L - 1))
+
+
+def test_normalize_rows_are_stochastic_and_edges_masked():
+    """Eq. (3): nonnegative, rows sum to one over N(j), out-of-grid taps are exactly 0
+    (vertical directions mask along j, horizontal ones along i)."""
+    rng = np.random.default_rng(30)
+    H, W = 5, 7
+    wt = rng.normal(0, 2, (4, 2, 3, 3, H, W))
+    w = orc.normalize(wt, 15)
+    assert np.all(w >= 0)
+    np.testing.assert_allclose(w.sum(axis=3), 1.0, atol=1e-14)
+    for d in range(4):
+        for k in range(3):
+            for i in range(H):
+                for j in range(W):
+                    if not _in_grid(d, k, i, j, H, W):
+                        assert np.all(w[d, :, :, k, i, j] == 0.0)
+                    else:
+                        assert np.all(w[d, :, :, k, i, j] > 0.0)
+
+
+def test_normalize_equal_logits_closed_form():
+    """Equal logits: every in-grid tap gets 1/|N(j)| (1/3 inside, 1/2 on an edge, 1 on a line of one)."""
+    for H, W in ((4, 6), (1, 5), (5, 1), (1, 1)):
+        for c in (-3.0, 0.0, 2.5):
+            w = orc.normalize(np.full((4, 1, 1, 3, H, W), c), 15)
+            for d in range(4):
+                for i in range(H):
+                    for j in range(W):
+                        n = sum(_in_grid(d, k, i, j, H, W) for k in range(3))
+                        for k in range(3):
+                            exp = 1.0 / n if _in_grid(d, k, i, j, H, W) else 0.0
+                            assert abs(w[d, 0, 0, k, i, j] - exp) < 1e-15
+
+
+def test_normalize_ratio_identity_with_library_softplus():
+    """log(w_k / w_k') = log sigmoid(a_k) - log sigmoid(a_k') = softplus(-a_k') - softplus(-a_k):
+    numpy's logaddexp gives the right-hand side without forming a sigmoid or a sum."""
+    rng = np.random.default_rng(31)
+    wt = rng.normal(0, 3, (1, 2, 2, 3, 6, 6))
+    w = orc.normalize(wt, 1)
+    inner = (slice(None),) * 3
+    lhs = np.log(w[inner + (0, slice(None), slice(1, 5))] / w[inner + (2, slice(None), slice(1, 5))])
+    a0 = wt[inner + (0, slice(None), slice(1, 5))]
+    a2 = wt[inner + (2, slice(None), slice(1, 5))]
+    rhs = np.logaddexp(0.0, -a2) - np.logaddexp(0.0, -a0)
+    np.testing.assert_allclose(lhs, rhs, atol=1e-12)
+
+
+def test_normalize_two_tap_edge_is_a_logistic_of_softplus_difference():
+    """On an edge N(j) has two taps: w_1 = 1 / (1 + sigmoid(a_2)/sigmoid(a_1)) = expit(softplus(-a_2) - softplus(-a_1))
+    with scipy's expit as the library routine."""
+    from scipy.special import expit
+    rng = np.random.default_rng(32)
+    wt = rng.normal(0, 2, (1, 1, 1, 3, 4, 5))
+    w = orc.normalize(wt, 1)                      # T->B: column 0 has no k=0 neighbour
+    a1, a2 = wt[0, 0, 0, 1, :, 0], wt[0, 0, 0, 2, :, 0]
+    np.testing.assert_allclose(w[0, 0, 0, 1, :, 0], expit(np.logaddexp(0, -a2) - np.logaddexp(0, -a1)), atol=1e-14)
+
+
+def test_normalize_clamp_branch_constant():
+    """All logits -40: S = 3*sigmoid(-40) = 1.27e-17 < eps = 1e-6, so w_k = sigmoid(-40)/eps.
+    sigmoid(-40) = e^-40/(1+e^-40) = 4.248354255291589e-18 (e^-40 to 16 digits)."""
+    w = orc.normalize(np.full((1, 1, 1, 3, 3, 3), -40.0), 1)
+    np.testing.assert_allclose(w[0, 0, 0, :, 1, 1], 4.248354255291589e-12, rtol=1e-12)
+    assert w[0, 0, 0, 0, 1, 0] == 0.0             # masking still applies under the clamp
+
+
+@pytest.mark.parametrize("mask", [1, 4, 15, 10])
+def test_normalize_bwd_finite_differences(mask):
+    """Central differences in fp64 of <dw3, normalize(wt)> against the adjoint, clamp inactive."""
+    rng = np.random.default_rng(33 + mask)
+    D = orc.popcount(mask)
+    wt = rng.normal(0, 1.5, (D, 1, 2, 3, 4, 5))
+    dw = rng.standard_normal(wt.shape)
+    g = orc.normalize_bwd(wt, dw, mask)
+    eps = 1e-6
+    idx = [tuple(rng.integers(0, n) for n in wt.shape) for _ in range(60)]
+    for ix in idx:
+        p, m = wt.copy(), wt.copy()
+        p[ix] += eps; m[ix] -= eps
+        fd = float(np.sum(dw * (orc.normalize(p, mask) - orc.normalize(m, mask)))) / (2 * eps)
+        assert abs(fd - g[ix]) <= 1e-8 + 1e-6 * abs(fd), (ix, fd, g[ix])
+
+
+def test_normalize_bwd_clamp_branch_and_invariants():
+    """(a) clamp active: the denominator is the constant eps, so dwt_k = s_k(1-s_k) dw_k / eps -- checked by
+    finite differences; (b) clamp inactive: rows of w sum to one, so a constant added to dw over N(j) changes
+    nothing; (c) out-of-grid taps get no gradient."""
+    rng = np.random.default_rng(35)
+    wt = np.full((1, 1, 1, 3, 3, 4), -40.0) + rng.normal(0, 0.1, (1, 1, 1, 3, 3, 4))
+    dw = rng.standard_normal(wt.shape)
+    g = orc.normalize_bwd(wt, dw, 1)
+    for ix in [(0, 0, 0, 1, 1, 1), (0, 0, 0, 0, 2, 2), (0, 0, 0, 2, 0, 1)]:
+        p, m = wt.copy(), wt.copy()
+        p[ix] += 1e-4; m[ix] -= 1e-4
+        fd = float(np.sum(dw * (orc.normalize(p, 1) - orc.normalize(m, 1)))) / 2e-4
+        assert abs(fd - g[ix]) <= 1e-6 * abs(fd) + 1e-30
+    wt = rng.normal(0, 1, (2, 1, 2, 3, 4, 5))
+    dw = rng.standard_normal(wt.shape)
+    g0 = orc.normalize_bwd(wt, dw, 5)
+    g1 = orc.normalize_bwd(wt, dw + 3.25, 5)
+    np.testing.assert_allclose(g0, g1, atol=1e-13)
+    assert np.all(g0[0, :, :, 0, :, 0] == 0) and np.all(g0[0, :, :, 2, :, -1] == 0)      # T->B: along j
+    assert np.all(g0[1, :, :, 0, 0, :] == 0) and np.all(g0[1, :, :, 2, -1, :] == 0)      # L->R: along i
+
+
+def test_normalized_taps_feed_the_scan_stably():
+    """Eq. (3) output used as w3: the stability bound of PAPER.md:94 holds (|h| <= M * sum of lambda maxima)."""
+    rng = np.random.default_rng(36)
+    B, C, H, W, G = 1, 4, 9, 8, 2
+    w3 = orc.normalize(rng.normal(0, 2, (4, B, G, 3, H, W)), 15)
+    x = rng.uniform(-1, 1, (B, C, H, W))
+    lam = rng.uniform(0, 1, (4, B, C, H, W))
+    y, h = orc.fwd(x, w3, lam, np.ones_like(lam), G, 15, return_h=True)
+    for q in range(4):
+        Ls = H if q < 2 else W
+        bound = lam[q].max() * Ls
+        assert np.all(np.abs(h[q]) <= bound + 1e-12)
