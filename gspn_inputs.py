@@ -32,7 +32,7 @@ import torch
 
 DIR_TB, DIR_BT, DIR_LR, DIR_RL, DIR_ALL = 1, 2, 4, 8, 15
 
-_T_X, _T_W, _T_LAM, _T_U, _T_DY, _T_H0 = 1, 2, 3, 4, 5, 6
+_T_X, _T_W, _T_LAM, _T_U, _T_DY, _T_H0, _T_DW = 1, 2, 3, 4, 5, 6, 7
 _MASK63 = (1 << 63) - 1
 
 
@@ -186,6 +186,27 @@ def make_inputs(cfg: ScanConfig, dtype: str, device="cpu", batch_slice=None,
         h0 = [_draw("normal", b0 * C * L, nb * C * L, cfg.seed, _T_H0, d, device).view(nb, C, L)
               for d in dirs]
         out["h0"] = torch.stack(h0).to(st).contiguous()
+    return out
+
+
+def make_logits(cfg: ScanConfig, dtype: str, device="cpu", batch_slice=None, with_dw: bool = False) -> dict:
+    """Raw tap logits wt [D,b,G,3,H,W] ~ N(0, logit_std) for the Eq. (3) normalisation (the same draws that
+    make_inputs turns into w3), optionally with an upstream gradient dw3 ~ N(0,1) of the same shape."""
+    B, G, H, W = cfg.B, cfg.G, cfg.H, cfg.W
+    b0, b1 = (0, B) if batch_slice is None else batch_slice
+    nb = b1 - b0
+    st = torch_dtype(dtype)
+    plane = H * W
+    wt, dw = [], []
+    for d in dir_list(cfg.dir_mask):
+        wt.append(_draw("normal", b0 * G * 3 * plane, nb * G * 3 * plane, cfg.seed, _T_W, d,
+                        device).view(nb, G, 3, H, W) * cfg.logit_std)
+        if with_dw:
+            dw.append(_draw("normal", b0 * G * 3 * plane, nb * G * 3 * plane, cfg.seed, _T_DW, d,
+                            device).view(nb, G, 3, H, W))
+    out = {"wt": torch.stack(wt).to(st).contiguous()}
+    if with_dw:
+        out["dw3"] = torch.stack(dw).to(st).contiguous()
     return out
 
 

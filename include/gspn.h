@@ -104,6 +104,23 @@ int gspn_scan_bwd(const void* x, const void* w3, const void* lambda, const void*
 int gspn_merge(const void* y_dirs, const float* m, void* y,
                int B, int C, int H, int W, unsigned dir_mask, int dtype, void* stream);
 
+/*
+ * Row-stochastic normalisation of the raw tap logits, Eq. (3), fused in one pass as the paper's
+ * normalisation kernel is ("sigmoid activation, local reduction, clamping, and division"):
+ *     s_k = sigmoid(wt[k]),   S = sum of s_k over the taps k whose neighbour lies inside the grid (N(j) of Eq. 3),
+ *     w3[k] = s_k / max(S, GSPN_NORM_EPS) for k in N(j),   0 for the out-of-grid taps
+ * (tap k <-> neighbour k-1 on the cross axis: j for T->B / B->T, i for L->R / R->L).  wt, w3: DEVICE pointers,
+ * [D,B,G,3,H,W] dense, storage type `dtype`, 16-byte aligned, w3 fully overwritten, must not alias wt; fp32
+ * arithmetic, one RNE per output.  The paper states no clamp bound: GSPN_NORM_EPS is DESIGN.md reading R17.
+ * gspn_normalize_bwd writes dwt = (d w3 / d wt)^T dw3 evaluated at wt (same layouts).  Asynchronous on `stream`;
+ * returns a GSPN_* status (GSPN_EINVAL / GSPN_EALIGN / GSPN_ECUDA as for the scans).
+ */
+#define GSPN_NORM_EPS 1e-6f
+int gspn_normalize_fwd(const void* wt, void* w3, int B, int G, int H, int W, unsigned dir_mask, int dtype,
+                       void* stream);
+int gspn_normalize_bwd(const void* wt, const void* dw3, void* dwt, int B, int G, int H, int W,
+                       unsigned dir_mask, int dtype, void* stream);
+
 /* Extended arguments: initial state and kernel selection. */
 typedef struct gspn_args {
     size_t struct_size;            /* = sizeof(gspn_args_t) */

@@ -138,8 +138,10 @@ int gspn_oracle_normalize_f64(const double *wt, double *w3, int B, int G, int H,
  *     dL/ds_k = dw_k / eps                                    where it is active (the denominator is a constant)
  * and dwt_k = 0 for the out-of-grid taps (they do not reach any output).
  */
+/* magnitude != 0: the sum of the absolute values of the terms instead (|dw| and a plus inside the bracket):
+ * the scale rounding errors of dwt are relative to (tests/parity_util.py). */
 int gspn_oracle_normalize_bwd_f64(const double *wt, const double *dw3, double *dwt, int B, int G, int H,
-                                  int W, unsigned mask, double eps)
+                                  int W, unsigned mask, double eps, int magnitude)
 {
     if (B < 1 || G < 1 || H < 1 || W < 1 || mask < 1 || mask > 15) return 1;
     const size_t plane = (size_t)H * W;
@@ -158,13 +160,16 @@ int gspn_oracle_normalize_bwd_f64(const double *wt, const double *dw3, double *d
                         v[k] = norm_valid(dir, k, i, j, H, W);
                         if (v[k]) S += s[k];
                     }
+                    double g[3];
+                    for (int k = 0; k < 3; ++k) g[k] = magnitude ? fabs(dw3[o + k * plane]) : dw3[o + k * plane];
                     double dot = 0.0;                      /* sum_k' dw_k' w_k' over N(j) */
                     if (S > eps)
                         for (int k = 0; k < 3; ++k)
-                            if (v[k]) dot += dw3[o + k * plane] * (s[k] / S);
+                            if (v[k]) dot += g[k] * (s[k] / S);
+                    if (magnitude) dot = -dot;
                     for (int k = 0; k < 3; ++k) {
                         double ds = 0.0;
-                        if (v[k]) ds = S > eps ? (dw3[o + k * plane] - dot) / S : dw3[o + k * plane] / eps;
+                        if (v[k]) ds = S > eps ? (g[k] - dot) / S : g[k] / eps;
                         dwt[o + k * plane] = s[k] * (1.0 - s[k]) * ds;
                     }
                 }

@@ -138,15 +138,15 @@ def normalize(wt, mask: int, eps: float = NORM_EPS):
     return w3
 
 
-def normalize_bwd(wt, dw3, mask: int, eps: float = NORM_EPS):
-    """dwt = adjoint of normalize at wt applied to dw3 (fp64)."""
+def normalize_bwd(wt, dw3, mask: int, eps: float = NORM_EPS, magnitude: bool = False):
+    """dwt = adjoint of normalize at wt applied to dw3 (fp64); magnitude=True: sum of |terms| instead."""
     wt = _prep(wt, np.float64)
     dw3 = _prep(dw3, np.float64)
     D, B, G, three, H, W = wt.shape
     assert three == 3 and D == popcount(mask) and dw3.shape == wt.shape
     dwt = np.empty_like(wt)
     rc = _load().gspn_oracle_normalize_bwd_f64(_ptr(wt), _ptr(dw3), _ptr(dwt), B, G, H, W,
-                                               ctypes.c_uint(mask), ctypes.c_double(eps))
+                                               ctypes.c_uint(mask), ctypes.c_double(eps), int(magnitude))
     if rc != 0:
         raise ValueError("gspn_oracle_normalize_bwd: invalid arguments")
     return dwt

@@ -22,7 +22,8 @@ STATUS = {0: "GSPN_OK", 1: "GSPN_EINVAL", 2: "GSPN_EUNSUPPORTED", 3: "GSPN_EALIG
           4: "GSPN_EWORKSPACE", 5: "GSPN_ECUDA"}
 
 EXPORTS = ("gspn_scan_fwd", "gspn_scan_bwd", "gspn_merge", "gspn_scan_fwd_ex", "gspn_scan_bwd_ex",
-           "gspn_scan_fwd_host", "gspn_scan_bwd_host", "gspn_workspace_bytes",
+           "gspn_scan_fwd_host", "gspn_scan_bwd_host", "gspn_normalize_fwd", "gspn_normalize_bwd",
+           "gspn_workspace_bytes",
            "gspn_last_launch_count", "gspn_last_variant", "gspn_last_error", "gspn_version")
 
 
@@ -59,6 +60,8 @@ def lib() -> ctypes.CDLL:
         L.gspn_scan_fwd.argtypes = [vp] * 5 + [ci] * 5 + [cu, ci, vp]
         L.gspn_scan_bwd.argtypes = [vp] * 10 + [ci] * 5 + [cu, ci, vp]
         L.gspn_merge.argtypes = [vp] * 3 + [ci] * 4 + [cu, ci, vp]
+        L.gspn_normalize_fwd.argtypes = [vp] * 2 + [ci] * 4 + [cu, ci, vp]
+        L.gspn_normalize_bwd.argtypes = [vp] * 3 + [ci] * 4 + [cu, ci, vp]
         L.gspn_scan_fwd_host.argtypes = L.gspn_scan_fwd.argtypes
         L.gspn_scan_bwd_host.argtypes = L.gspn_scan_bwd.argtypes
         L.gspn_scan_fwd_ex.argtypes = [ctypes.POINTER(_Args)]
@@ -180,6 +183,37 @@ def gspn_merge(y_dirs, m=None, dir_mask: int = DIR_ALL, out=None):
                               _stream(y_dirs))
     _check(rc)
     return y
+
+
+def _norm_shape(wt, dir_mask):
+    if not wt.is_cuda or not wt.is_contiguous() or wt.dim() != 6 or wt.shape[3] != 3:
+        raise ValueError("wt: need a contiguous CUDA tensor [D,B,G,3,H,W] (there is no CPU path)")
+    D, B, G, _, H, W = wt.shape
+    if D != _popcount(dir_mask):
+        raise ValueError(f"wt: {D} direction slabs but dir_mask={dir_mask}")
+    return B, G, H, W
+
+
+def gspn_normalize_fwd(wt, dir_mask: int = DIR_ALL, out=None):
+    """w3 = Eq. (3) of the tap logits wt [D,B,G,3,H,W]; see include/gspn.h gspn_normalize_fwd."""
+    B, G, H, W = _norm_shape(wt, dir_mask)
+    w3 = torch.empty_like(wt) if out is None else _dev(out, "out", wt.shape, wt)
+    with torch.cuda.device(wt.device):
+        rc = lib().gspn_normalize_fwd(_p(wt), _p(w3), B, G, H, W, dir_mask, _dtype_code(wt), _stream(wt))
+    _check(rc)
+    return w3
+
+
+def gspn_normalize_bwd(wt, dw3, dir_mask: int = DIR_ALL, out=None):
+    """dwt = adjoint of gspn_normalize_fwd at wt applied to dw3; see include/gspn.h gspn_normalize_bwd."""
+    B, G, H, W = _norm_shape(wt, dir_mask)
+    _dev(dw3, "dw3", wt.shape, wt)
+    dwt = torch.empty_like(wt) if out is None else _dev(out, "out", wt.shape, wt)
+    with torch.cuda.device(wt.device):
+        rc = lib().gspn_normalize_bwd(_p(wt), _p(dw3), _p(dwt), B, G, H, W, dir_mask, _dtype_code(wt),
+                                      _stream(wt))
+    _check(rc)
+    return dwt
 
 
 def _host(t, name):

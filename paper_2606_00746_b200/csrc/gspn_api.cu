@@ -180,6 +180,35 @@ int gspn_merge(const void* y_dirs, const float* m, void* y,
     return rc;
 }
 
+int gspn_normalize_fwd(const void* wt, void* w3, int B, int G, int H, int W, unsigned dir_mask, int dtype,
+                       void* stream) {
+    int rc = check_shape(B, G, H, W, G, dir_mask, dtype);
+    if (rc) return rc;
+    REQUIRE_PTR(wt); REQUIRE_PTR(w3);
+    LaunchInfo li{0, ""};
+    rc = dtype == GSPN_F32
+             ? norm_launch<float>((const float*)wt, nullptr, (float*)w3, B, G, H, W, dir_mask, (cudaStream_t)stream, &li)
+             : norm_launch<__nv_bfloat16>((const __nv_bfloat16*)wt, nullptr, (__nv_bfloat16*)w3, B, G, H, W, dir_mask,
+                                          (cudaStream_t)stream, &li);
+    if (rc == GSPN_OK) { g_launches = li.launches; g_variant = li.variant; }
+    return rc;
+}
+
+int gspn_normalize_bwd(const void* wt, const void* dw3, void* dwt, int B, int G, int H, int W,
+                       unsigned dir_mask, int dtype, void* stream) {
+    int rc = check_shape(B, G, H, W, G, dir_mask, dtype);
+    if (rc) return rc;
+    REQUIRE_PTR(wt); REQUIRE_PTR(dw3); REQUIRE_PTR(dwt);
+    LaunchInfo li{0, ""};
+    rc = dtype == GSPN_F32
+             ? norm_launch<float>((const float*)wt, (const float*)dw3, (float*)dwt, B, G, H, W, dir_mask,
+                                  (cudaStream_t)stream, &li)
+             : norm_launch<__nv_bfloat16>((const __nv_bfloat16*)wt, (const __nv_bfloat16*)dw3, (__nv_bfloat16*)dwt, B, G,
+                                          H, W, dir_mask, (cudaStream_t)stream, &li);
+    if (rc == GSPN_OK) { g_launches = li.launches; g_variant = li.variant; }
+    return rc;
+}
+
 // ---- host-pointer entry points ------------------------------------------------------------
 #define CUDA_TRY(expr)                                                                   \
     do {                                                                                 \

@@ -34,6 +34,11 @@ template <typename ST>
 int merge_launch(const ST* y_dirs, const float* m, ST* y, int D, int B, int C, int H, int W,
                  cudaStream_t st, LaunchInfo* li);
 
+// Eq. 3 normalisation of the tap logits and its adjoint (gspn_norm.cu); dw3 == nullptr selects the forward
+template <typename ST>
+int norm_launch(const ST* wt, const ST* dw3, ST* out, int B, int G, int H, int W, unsigned mask,
+                cudaStream_t st, LaunchInfo* li);
+
 void set_error(const char* fmt, ...);
 
 }  // namespace gspn

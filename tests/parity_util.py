@@ -147,3 +147,29 @@ def check_bwd_sampled(cfg: gi.ScanConfig, dtype: str, tensors: dict, grads: dict
             res["ok"] = res["ok"] and entry[k]["ok"]
         res["slices"].append(entry)
     return res
+
+
+# ---- Eq. (3) normalisation ------------------------------------------------------------
+def norm_bwd_magnitude(wt: np.ndarray, dw3: np.ndarray, mask: int) -> np.ndarray:
+    """Sum of the absolute values of the terms behind dwt (the oracle's magnitude run)."""
+    return orc.normalize_bwd(wt, dw3, mask, magnitude=True)
+
+
+def check_norm(cfg: gi.ScanConfig, dtype: str, device: str = "cuda:0", batch_slice=None, backward: bool = True) -> dict:
+    """Whole-tensor parity of gspn_normalize_fwd / _bwd through the C ABI against the fp64 oracle."""
+    import paper_2606_00746_b200 as gspn
+    t = gi.make_logits(cfg, dtype, device="cpu", batch_slice=batch_slice, with_dw=backward)
+    d = {k: v.to(device) for k, v in t.items()}
+    w3 = gspn.gspn_normalize_fwd(d["wt"], cfg.dir_mask)
+    variant = gspn.gspn_last_variant()
+    wt64 = np64(t["wt"])
+    ref = orc.normalize(wt64, cfg.dir_mask)
+    out = {"fwd": gate(np64(w3), ref, np.abs(ref), dtype), "variant": variant}
+    out["ok"] = out["fwd"]["ok"]
+    if backward:
+        dwt = gspn.gspn_normalize_bwd(d["wt"], d["dw3"], cfg.dir_mask)
+        dw64 = np64(t["dw3"])
+        gref = orc.normalize_bwd(wt64, dw64, cfg.dir_mask)
+        out["bwd"] = gate(np64(dwt), gref, norm_bwd_magnitude(wt64, dw64, cfg.dir_mask), dtype)
+        out["ok"] = bool(out["ok"] and out["bwd"]["ok"])
+    return out

@@ -265,3 +265,63 @@ def test_chain_kernels_random_shapes():
             ran += 1
             assert r["ok"], (check.__name__, impl, (B, C, H, W, G), mask, dt, h0, r)
     assert ran >= 60
+
+
+# ---- Eq. (3) normalisation ------------------------------------------------------------
+NORM_SHAPES = [(1, 1, 1, 1, 1), (1, 2, 1, 5, 2), (2, 2, 5, 1, 1), (2, 4, 5, 7, 2), (1, 8, 16, 16, 8), (2, 4, 27, 27, 2),
+               (1, 4, 73, 73, 1), (2, 8, 56, 56, 4), (1, 2, 128, 128, 2), (1, 2, 64, 130, 1), (1, 3, 300, 37, 3)]
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("shape", NORM_SHAPES, ids=_ids(NORM_SHAPES))
+def test_normalize_small_shapes(shape, dtype):
+    """gspn_normalize_fwd / _bwd against the fp64 oracle: vector path (16-byte-aligned planes) and scalar
+    path (odd H*W in bf16), lines of one, ragged tails, every direction's edge mask."""
+    if shape[0] * shape[4] * shape[2] * shape[3] <= 8 and dtype == "bf16":
+        pytest.skip("the relative-L2 gate is not meaningful for a handful of elements")
+    cfg = gi.small_config("nz", *shape, seed=41)
+    r = pu.check_norm(cfg, dtype)
+    assert r["ok"], r
+
+
+@pytest.mark.parametrize("mask", [1, 2, 4, 8, 5, 10, 14])
+def test_normalize_direction_masks_and_sharp_logits(mask):
+    """Each direction slab masks its own cross axis; logit std 6 drives sigmoids to both tails."""
+    import dataclasses
+    for dtype in ("f32", "bf16"):
+        cfg = dataclasses.replace(gi.small_config("nm", 2, 4, 9, 12, 2, dir_mask=mask, seed=50 + mask), logit_std=6.0)
+        r = pu.check_norm(cfg, dtype)
+        assert r["ok"], (dtype, r)
+
+
+def test_normalize_clamp_branch_on_gpu():
+    """All logits near -40: S < GSPN_NORM_EPS, the clamp is active in forward and backward."""
+    wt = torch.full((1, 1, 2, 3, 6, 8), -40.0, device="cuda:0") + 0.25 * torch.randn(
+        (1, 1, 2, 3, 6, 8), generator=torch.Generator().manual_seed(3)).cuda()
+    dw = torch.randn(wt.shape, generator=torch.Generator().manual_seed(4)).cuda()
+    w3 = gspn.gspn_normalize_fwd(wt, 1)
+    dwt = gspn.gspn_normalize_bwd(wt, dw, 1)
+    ref = pu.orc.normalize(pu.np64(wt), 1)
+    gref = pu.orc.normalize_bwd(pu.np64(wt), pu.np64(dw), 1)
+    assert np.all(np.abs(pu.np64(w3) - ref) <= 1e-5 * np.abs(ref) + 1e-30)
+    assert np.all(np.abs(pu.np64(dwt) - gref) <= 2e-5 * np.abs(gref) + 1e-30)
+
+
+@pytest.mark.parametrize("name,dtype", [("cfg5_1k", "bf16"), ("cfg4_2k", "bf16"), ("cfg2_cls56", "f32")])
+def test_normalize_full_size_configs(name, dtype):
+    """The launch bench.py times (whole batch), checked on the first / middle / last images."""
+    cfg = gi.CONFIGS[name]
+    t = gi.make_logits(cfg, dtype, device="cuda:0", with_dw=True)
+    w3 = gspn.gspn_normalize_fwd(t["wt"], cfg.dir_mask)
+    dwt = gspn.gspn_normalize_bwd(t["wt"], t["dw3"], cfg.dir_mask)
+    for b in (0, cfg.B // 2, cfg.B - 1):
+        wt64, dw64 = pu.np64(t["wt"][:, b:b + 1]), pu.np64(t["dw3"][:, b:b + 1])
+        ref = pu.orc.normalize(wt64, cfg.dir_mask)
+        r = pu.gate(pu.np64(w3[:, b:b + 1]), ref, np.abs(ref), dtype)
+        assert r["ok"], (b, r)
+        gref = pu.orc.normalize_bwd(wt64, dw64, cfg.dir_mask)
+        r = pu.gate(pu.np64(dwt[:, b:b + 1]), gref, pu.norm_bwd_magnitude(wt64, dw64, cfg.dir_mask), dtype)
+        assert r["ok"], (b, r)
+    # rows of the normalised taps sum to one up to the storage rounding: a property that holds at any size
+    s = w3.float().sum(dim=3)
+    assert float((s - 1).abs().max()) <= (1.2e-2 if dtype == "bf16" else 1e-5)
