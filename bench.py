@@ -421,6 +421,30 @@ def main():
                                                "pxch_per_s": oc.n / (r["fwd_ms_mean"] * 1e-3)}
                 del tt, yy, gg
                 torch.cuda.empty_cache()
+        # the fused Eq. 3 normalisation of the tap logits and its adjoint on every config
+        # (algorithmic bytes: logits read + taps written = 2 D n_w s; backward reads logits and dw3, writes dwt = 3 D n_w s)
+        for name, oc in gi.CONFIGS.items():
+            for dt in oc.dtypes:
+                so = 4 if dt == "f32" else 2
+                lg = gi.make_logits(oc, dt, device=torch.device("cuda", torch.cuda.current_device()), with_dw=True)
+                buf = torch.empty_like(lg["wt"])
+                for tag, fn, nbytes in (("norm_fwd", lambda: gspn.gspn_normalize_fwd(lg["wt"], oc.dir_mask, out=buf), 2),
+                                        ("norm_bwd", lambda: gspn.gspn_normalize_bwd(lg["wt"], lg["dw3"], oc.dir_mask, out=buf), 3)):
+                    for _ in range(3):
+                        fn()
+                    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+                    nrep = max(5, min(steps, 20))
+                    ev[0].record()
+                    for _ in range(nrep):
+                        fn()
+                    ev[1].record()
+                    torch.cuda.synchronize()
+                    ms = ev[0].elapsed_time(ev[1]) / nrep
+                    nb = nbytes * oc.D * oc.n_w * so
+                    others[f"{name}:{dt}:{tag}"] = {"variant": gspn.gspn_last_variant(), "ms": ms,
+                                                    "gbs": nb / (ms * 1e-3) / 1e9, "frac": nb / (ms * 1e-3) / 1e9 / peak}
+                del lg, buf
+                torch.cuda.empty_cache()
 
     cpu = None
     if not args.no_cpu and rank == 0 and world == 1:
