@@ -16,8 +16,8 @@ pytestmark = pytest.mark.gpu
 
 IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO]
 IMPL_IDS = ["naive", "auto"]
-FWD_IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO, gspn.IMPL_FLAT, gspn.IMPL_CHAIN, gspn.IMPL_PAIR]
-FWD_IMPL_IDS = ["naive", "auto", "flat", "chain", "pair"]
+FWD_IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO, gspn.IMPL_FLAT, gspn.IMPL_CHAIN, gspn.IMPL_PAIR, gspn.IMPL_PLANE]
+FWD_IMPL_IDS = ["naive", "auto", "flat", "chain", "pair", "plane"]
 
 # (B, C, H, W, G): degenerate lines, W in {1,2,3}, H != W, beyond one warp, ragged tails, cg in {1,C}
 SMALL_SHAPES = [
@@ -33,11 +33,11 @@ def _ids(shapes):
 
 
 def _fwd_or_skip(impl, fn):
-    """The pair kernel keeps whole fp32 planes on chip: shapes it reports as unsupported are skipped."""
+    """The pair / plane kernels keep whole fp32 planes on chip: shapes they report as unsupported are skipped."""
     try:
         return fn()
     except gspn.GspnError as ex:
-        if impl == gspn.IMPL_PAIR and ex.status == 2:          # GSPN_EUNSUPPORTED
+        if impl in (gspn.IMPL_PAIR, gspn.IMPL_PLANE) and ex.status == 2:          # GSPN_EUNSUPPORTED
             pytest.skip(str(ex))
         raise
 
@@ -47,7 +47,7 @@ def _fwd_or_skip(impl, fn):
 @pytest.mark.parametrize("shape", SMALL_SHAPES, ids=_ids(SMALL_SHAPES))
 def test_fwd_small_shapes(shape, dtype, impl):
     cfg = gi.small_config("s", *shape, seed=11)
-    if impl in (gspn.IMPL_CHAIN, gspn.IMPL_PAIR) and max(shape[2], shape[3]) > 128:
+    if impl in (gspn.IMPL_CHAIN, gspn.IMPL_PAIR, gspn.IMPL_PLANE) and max(shape[2], shape[3]) > 128:
         pytest.skip("chain kernels hold lines of at most 128 positions")
     r = _fwd_or_skip(impl, lambda: pu.check_fwd(cfg, dtype, impl=impl))
     assert r["ok"], r
@@ -238,6 +238,11 @@ def test_auto_selects_fused_kernels_where_supported():
     assert gspn.gspn_last_launch_count() == 1
     r = pu.check_fwd(cfg, "bf16")
     assert r["ok"] and r["variant"] == "chain_fwd", r
+    # 378-px kind of shape (27x27, rows not 16-byte aligned, lines of one warp): the whole-plane kernel
+    cfg = gi.small_config("sel27", 2, 8, 27, 27, 2, seed=10)
+    r = pu.check_fwd(cfg, "bf16")
+    assert r["ok"] and r["variant"] == "plane_fwd", r
+
 
 def test_chain_kernels_random_shapes():
     """Seeded sweep of the chain kernels and the pair forward kernel (forced) over random shapes, masks, dtypes, group sizes and
@@ -255,7 +260,7 @@ def test_chain_kernels_random_shapes():
         if B * C * H * W <= 8 and dt == "bf16":
             continue        # the relative-L2 gate is not meaningful for a handful of elements
         cfg = gi.small_config("rz", B, C, H, W, G, dir_mask=mask, seed=3000 + it, backward=True)
-        for check, impl in ((pu.check_fwd, gspn.IMPL_CHAIN), (pu.check_bwd, gspn.IMPL_CHAIN), (pu.check_fwd, gspn.IMPL_PAIR)):
+        for check, impl in ((pu.check_fwd, gspn.IMPL_CHAIN), (pu.check_bwd, gspn.IMPL_CHAIN), (pu.check_fwd, gspn.IMPL_PAIR), (pu.check_fwd, gspn.IMPL_PLANE)):
             try:
                 r = check(cfg, dt, impl=impl, with_h0=h0)
             except gspn.GspnError as ex:
@@ -264,7 +269,7 @@ def test_chain_kernels_random_shapes():
                 raise
             ran += 1
             assert r["ok"], (check.__name__, impl, (B, C, H, W, G), mask, dt, h0, r)
-    assert ran >= 60
+    assert ran >= 70
 
 
 # ---- Eq. (3) normalisation ------------------------------------------------------------
