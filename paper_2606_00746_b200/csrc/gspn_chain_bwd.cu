@@ -392,12 +392,19 @@ __device__ __forceinline__ void chain_bwd_out(const ChainBwdParams& p, uint8_t* 
             for (int c = 0; c < NS; ++c) {
                 const uint32_t hc = hb0 + (uint32_t)c * 2 * (kBlk + 1) * P * 128 + hoff;
                 const uint32_t gc = gb0 + (uint32_t)c * 2 * kBlk * P * 128 + goff;
-                float hn[P], hp[P], gh[P];
+                float hn[P], hp[P], gh[P], dxo[P];
+                uint32_t dxa[P];
 #pragma unroll
                 for (int e = 0; e < P; ++e) {
                     hp[e] = lds32(hc + e * 128);
                     hn[e] = lds32(hc + (P + e) * 128);
                     gh[e] = lds32(gc + e * 128);
+                    // the dx accumulators of this step are read together with the block buffers: one shared-memory
+                    // round trip per channel instead of a read -> write -> read chain per position
+                    if constexpr (!VH) dxa[e] = dxs + (((uint32_t)c * H + li) * p.Wp + P * lane + e) * 4;
+                    else dxa[e] = dxs + (uint32_t)c * H * p.Wp * 4 + rowdx[e] + li * 4;
+                    dxo[e] = 0.f;
+                    if (w_dx && ok[e]) dxo[e] = lds32(dxa[e]);
                 }
                 const float hpl = maskf(lds32(hc + (P - 1) * 128 - 4), m_first);     // h[s-1] of position p-1 (lane-1)
                 const float hpr = maskf(lds32(hc + 4), m_31);                        // h[s-1] of position p+1 (lane+1)
@@ -436,17 +443,11 @@ __device__ __forceinline__ void chain_bwd_out(const ChainBwdParams& p, uint8_t* 
                         const size_t o = (size_t)c * HW + (size_t)li * W + P * lane + e;
                         if (w_du && ok[e]) E::stg(du0 + o, duv);
                         if (w_dl && ok[e]) E::stg(dl0 + o, dlv);
-                        if (w_dx && ok[e]) {
-                            const uint32_t a = dxs + (((uint32_t)c * H + li) * p.Wp + P * lane + e) * 4;
-                            sts32(a, fmaf(E::f(lr[e]), gh[e], lds32(a)));
-                        }
+                        if (w_dx && ok[e]) sts32(dxa[e], fmaf(E::f(lr[e]), gh[e], dxo[e]));
                     } else {
                         if (w_du && ok[e]) E::sts(tile + c * tplane + rowtl[e] + cs, duv);
                         if (w_dl && ok[e]) E::sts(tile + (NS + c) * tplane + rowtl[e] + cs, dlv);
-                        if (w_dx && ok[e]) {
-                            const uint32_t a = dxs + (uint32_t)c * H * p.Wp * 4 + rowdx[e] + li * 4;
-                            sts32(a, fmaf(E::f(lr[e]), gh[e], lds32(a)));
-                        }
+                        if (w_dx && ok[e]) sts32(dxa[e], fmaf(E::f(lr[e]), gh[e], dxo[e]));
                     }
                 }
             }

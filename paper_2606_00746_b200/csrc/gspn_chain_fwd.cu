@@ -150,11 +150,20 @@ __device__ __forceinline__ void chain_fwd_dir(const ChainFwdParams& p, uint8_t* 
                     acc = E::fma2(lr[e], xr[e], acc);
                     hn[e] = maskf(acc, okm[e]);                         // positions past the line stay +0
                 }
+                // Y += u*h: the step's reads first, then its writes (one shared-memory round trip per step
+                // instead of a read -> write -> read chain per position)
+                float yo[P];
 #pragma unroll
                 for (int e = 0; e < P; ++e) {
                     h[e] = hn[e];
                     const uint32_t a = VH ? yh[e] + (BLK * bi + tl) * 4 : yv + (tl * p.Wp + e) * 4;
-                    if (ok[e]) sts32(a, fmaf(E::f(ur[e]), hn[e], lds32(a)));
+                    yo[e] = 0.f;
+                    if (ok[e]) yo[e] = lds32(a);
+                }
+#pragma unroll
+                for (int e = 0; e < P; ++e) {
+                    const uint32_t a = VH ? yh[e] + (BLK * bi + tl) * 4 : yv + (tl * p.Wp + e) * 4;
+                    if (ok[e]) sts32(a, fmaf(E::f(ur[e]), hn[e], yo[e]));
                 }
             }
         }
