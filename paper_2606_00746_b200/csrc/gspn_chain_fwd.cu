@@ -334,8 +334,13 @@ chain_fwd_kernel(const ChainFwdParams p) {
         const float* Y = reinterpret_cast<const float*>(smem + p.off_y);
         ST* yg = reinterpret_cast<ST*>(p.y) + ((size_t)b * sh.C + c0) * HW;
         const int nw = blockDim.x >> 5;
-        for (int ci = warp; ci < NC * H; ci += nw)
-            for (int j = lane; j < W; j += 32) st_f(yg + (size_t)ci * W + j, Y[(size_t)ci * p.Wp + j]);
+        if (p.Wp == W) {       // odd W: Y has the pitch of the image rows, the CTA's planes are one contiguous run
+            const int total = NC * H * W;
+            for (int idx = threadIdx.x; idx < total; idx += blockDim.x) st_f(yg + idx, Y[idx]);
+        } else {
+            for (int ci = warp; ci < NC * H; ci += nw)
+                for (int j = lane; j < W; j += 32) st_f(yg + (size_t)ci * W + j, Y[(size_t)ci * p.Wp + j]);
+        }
     }
 }
 

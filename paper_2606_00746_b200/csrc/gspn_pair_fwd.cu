@@ -488,8 +488,13 @@ pair_fwd_kernel(const PairFwdParams p) {
     {
         const float* Y = reinterpret_cast<const float*>(smem + p.off_y);
         ST* yg = reinterpret_cast<ST*>(p.y) + ((size_t)b * sh.C + c0) * HW;
-        for (int ci = warp; ci < NC * H; ci += 4)
-            for (int j = lane; j < W; j += 32) st_f(yg + (size_t)ci * W + j, Y[(size_t)ci * p.Wp + j]);
+        if (p.Wp == W) {       // odd W: Y has the pitch of the image rows, the CTA's planes are one contiguous run
+            const int total = NC * H * W;
+            for (int idx = threadIdx.x; idx < total; idx += 128) st_f(yg + idx, Y[idx]);
+        } else {
+            for (int ci = warp; ci < NC * H; ci += 4)
+                for (int j = lane; j < W; j += 32) st_f(yg + (size_t)ci * W + j, Y[(size_t)ci * p.Wp + j]);
+        }
     }
 }
 
@@ -589,9 +594,16 @@ plane_fwd_kernel(const PairFwdParams p) {
         const float* Yv = reinterpret_cast<const float*>(smem + p.off_y);
         const float* Yh = reinterpret_cast<const float*>(smem + p.off_y2);
         ST* yg = reinterpret_cast<ST*>(p.y) + ((size_t)b * sh.C + c0) * HW;
-        for (int ci = warp; ci < NC * H; ci += NCMP + 1)
-            for (int j = lane; j < W; j += 32)
-                st_f(yg + (size_t)ci * W + j, Yv[(size_t)ci * p.Wp + j] + Yh[(size_t)ci * p.Wp + j]);
+        if (p.Wp == W) {
+            // odd W: the Y planes have the pitch of the image rows, so the CTA's NC output planes are one
+            // contiguous run both on chip and in HBM
+            const int total = NC * H * W;
+            for (int idx = threadIdx.x; idx < total; idx += 32 * (NCMP + 1)) st_f(yg + idx, Yv[idx] + Yh[idx]);
+        } else {
+            for (int ci = warp; ci < NC * H; ci += NCMP + 1)
+                for (int j = lane; j < W; j += 32)
+                    st_f(yg + (size_t)ci * W + j, Yv[(size_t)ci * p.Wp + j] + Yh[(size_t)ci * p.Wp + j]);
+        }
     }
 }
 
