@@ -55,6 +55,13 @@ def test_argument_validation_without_gpu(L):
     assert fwd(x=odd) == 3 and b"aligned" in L.gspn_last_error()
     assert L.gspn_scan_bwd(p, p, p, p, None, p, p, p, p, p, 1, 4, 4, 4, 2, 15, 0, None) == 1
     assert L.gspn_merge(None, None, p, 1, 4, 4, 4, 15, 0, None) == 1
+    # Eq. 3 normalisation: same validation rules
+    assert L.gspn_normalize_fwd(p, p, 0, 2, 4, 4, 15, 0, None) == 1
+    assert L.gspn_normalize_fwd(p, p, 1, 2, 4, 4, 0, 0, None) == 1
+    assert L.gspn_normalize_fwd(None, p, 1, 2, 4, 4, 15, 0, None) == 1 and b"NULL" in L.gspn_last_error()
+    assert L.gspn_normalize_fwd(p, odd, 1, 2, 4, 4, 15, 1, None) == 3
+    assert L.gspn_normalize_bwd(p, None, p, 1, 2, 4, 4, 15, 0, None) == 1
+    assert L.gspn_normalize_bwd(p, p, p, 1, 2, 4, 4, 15, 9, None) == 1
     # a backward call that asks for no output is a no-op
     assert L.gspn_scan_bwd(p, p, p, p, p, None, None, None, None, None, 1, 4, 4, 4, 2, 15, 0, None) == 0
     assert L.gspn_last_launch_count() == 0
