@@ -94,11 +94,15 @@ static int bwd_typed(const gspn_args_t* a) {
         rc = fused_bwd_launch<ST>(f, st, &li);
     } else if (a->impl == GSPN_IMPL_CHAIN) {
         rc = chain_bwd_launch<ST>(f, st, &li);
+    } else if (a->impl == GSPN_IMPL_PLANE) {
+        rc = plane_bwd_launch<ST>(f, st, &li);
     } else {
-        // lines of at most one warp (378-px config: 27x27): the per-block hand-shakes of the chain kernel cost
-        // more than the group kernel's block barriers (measured: cfg3 2.45 ms group, 2.97 ms chain)
+        // lines of at most one warp (378-px config: 27x27): the whole-plane kernel where the unit's planes fit on chip
+        // (cfg3 1.09 ms), else the group kernel (2.45 ms; the per-block hand-shakes of the chain kernel cost more
+        // there: 2.97 ms); longer lines: the chain kernel
         const bool small = f.sh.Lmax() <= 32;
-        rc = small ? fused_bwd_launch<ST>(f, st, &li) : chain_bwd_launch<ST>(f, st, &li);
+        rc = small ? plane_bwd_launch<ST>(f, st, &li) : chain_bwd_launch<ST>(f, st, &li);
+        if (rc == GSPN_EUNSUPPORTED && small) rc = fused_bwd_launch<ST>(f, st, &li);
         if (rc == GSPN_EUNSUPPORTED) rc = small ? chain_bwd_launch<ST>(f, st, &li) : fused_bwd_launch<ST>(f, st, &li);
         if (rc == GSPN_EUNSUPPORTED) rc = naive_bwd_launch<ST>(f, st, &li);
     }

@@ -31,6 +31,9 @@ template <typename ST> int pair_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st
 // whole-plane variant of the same for small planes (max(H,W) <= 64 and two CTAs' planes per SM): no rings
 template <typename ST> int plane_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 
+// whole-plane backward for small planes (gspn_plane_bwd.cu): lines of at most one warp, C/G in {1, 2, 4}
+template <typename ST> int plane_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
+
 // merge (gspn_merge.cu)
 template <typename ST>
 int merge_launch(const ST* y_dirs, const float* m, ST* y, int D, int B, int C, int H, int W,

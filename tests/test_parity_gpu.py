@@ -136,6 +136,31 @@ def test_bwd_chain_direction_masks_and_h0(mask):
     assert r["ok"], r
 
 
+PLANE_BWD_SHAPES = [(1, 1, 1, 1, 1), (1, 2, 1, 5, 1), (1, 2, 5, 1, 2), (1, 4, 8, 8, 2), (2, 4, 5, 7, 2), (2, 4, 7, 5, 4),
+                    (1, 4, 27, 27, 1), (2, 8, 27, 27, 2), (1, 4, 32, 32, 2), (1, 2, 20, 31, 1), (1, 8, 16, 16, 8)]
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("shape", PLANE_BWD_SHAPES, ids=_ids(PLANE_BWD_SHAPES))
+def test_bwd_plane_small_shapes(shape, dtype):
+    """Whole-plane backward kernel forced: lines of at most one warp, 1 / 2 / 4 channels per group, h0."""
+    if shape[0] * shape[1] * shape[2] * shape[3] <= 16 and dtype == "bf16":
+        pytest.skip("the relative-L2 gate is not meaningful for a handful of elements (every kernel, the naive one "
+                    "included, scores the same 3.2e-3 on this case's 10-element dh0)")
+    cfg = gi.small_config("pb", *shape, seed=23, backward=True)
+    r = _chain_or_skip(lambda: pu.check_bwd(cfg, dtype, impl=gspn.IMPL_PLANE, with_h0=True))
+    assert r["ok"], r
+    assert r["variant"] == "plane_bwd"
+
+
+@pytest.mark.parametrize("mask", [1, 2, 4, 8, 3, 12, 6, 9, 13, 15])
+def test_bwd_plane_direction_masks(mask):
+    cfg = gi.small_config("pbm", 2, 8, 11, 14, 2, dir_mask=mask, seed=70 + mask, backward=True)
+    for dtype in ("f32", "bf16"):
+        r = pu.check_bwd(cfg, dtype, impl=gspn.IMPL_PLANE, with_h0=(mask % 2 == 1))
+        assert r["ok"], (dtype, r)
+
+
 def test_bwd_optional_outputs():
     cfg = gi.small_config("opt", 1, 4, 8, 8, 2, seed=3, backward=True)
     t = {k: v.cuda() for k, v in gi.make_inputs(cfg, "f32").items()}
