@@ -251,6 +251,7 @@ plane_bwd_kernel(const PlaneBwdParams p) {
         if (warp == 1 && act[1]) plane_bwd_dir<ST, NC, false, true>(p, smem, 1, b, g, lane, act[0]);
         if (warp == 2 && act[2]) plane_bwd_dir<ST, NC, true, false>(p, smem, 2, b, g, lane, act[3]);
         if (warp == 3 && act[3]) plane_bwd_dir<ST, NC, true, true>(p, smem, 3, b, g, lane, act[2]);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // the in-place outputs, before the bulk stores read them
     }
     __syncthreads();
 
@@ -268,17 +269,31 @@ plane_bwd_kernel(const PlaneBwdParams p) {
                     st_f(dxg + (size_t)ci * W + j, dv[(size_t)ci * p.Wp + j] + dh[(size_t)ci * p.Wp + j]);
         }
     }
-    // du / dlambda / dw3 lie where u / lambda / the taps lay (same byte phase as in HBM: same tensor offsets)
+    // du / dlambda / dw3 lie where u / lambda / the taps lay, at the byte phase they have in HBM (same tensor
+    // offsets): the 16-byte-aligned interior of a plane leaves by ONE bulk store, the few elements before and
+    // after it by ordinary stores
     for (int pl = warp; pl < 4 * NP; pl += 5) {
         const int d = pl / NP, k = pl % NP;
         if (!act[d]) continue;
         ST* out = k < 3 ? reinterpret_cast<ST*>(p.dw3) : (k < 3 + NC ? reinterpret_cast<ST*>(p.dlam) : reinterpret_cast<ST*>(p.du));
         if (!out) continue;
         const unsigned long long b0 = pb_plane<NC, ES>(p, p.q[d], b, g, k).b0;
-        const ST* src = reinterpret_cast<const ST*>(smem + p.off_pl + (size_t)pl * p.plslot + (b0 & 15ull));
-        ST* dst = out + b0 / ES;
-        for (int idx = lane; idx < hw; idx += 32) dst[idx] = src[idx];
+        const uint32_t phase = (uint32_t)(b0 & 15ull), hwb = (uint32_t)hw * ES;
+        const uint32_t head = min((16u - phase) & 15u, hwb);                 // bytes before the aligned interior
+        const uint32_t inner = (hwb - head) & ~15u;
+        const uint8_t* src = smem + p.off_pl + (size_t)pl * p.plslot + phase;
+        uint8_t* dst = reinterpret_cast<uint8_t*>(out) + b0;
+        if (lane == 0 && inner > 0)
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst + head),
+                         "r"(smem_u32(src + head)), "r"(inner) : "memory");
+        for (uint32_t o = lane * ES; o < head; o += 32 * ES)
+            *reinterpret_cast<ST*>(dst + o) = *reinterpret_cast<const ST*>(src + o);
+        for (uint32_t o = head + inner + lane * ES; o < hwb; o += 32 * ES)
+            *reinterpret_cast<ST*>(dst + o) = *reinterpret_cast<const ST*>(src + o);
     }
+    // shared memory must outlive the bulk stores' reads
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 
 // ---- host side -----------------------------------------------------------------------------------
