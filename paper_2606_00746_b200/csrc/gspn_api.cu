@@ -66,9 +66,10 @@ static int fwd_typed(const gspn_args_t* a) {
         rc = plane_fwd_launch<ST>(f, st, &li);
     } else {
         rc = fused_fwd_launch<ST>(f, st, &li);
-        // rows that are not 16-byte aligned: lines of at most one warp whose planes fit on chip whole go to the
-        // whole-plane kernel (378-px config: 0.33 ms against 0.50 ms for the chain kernel), the rest to the chain kernel
-        if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO && f.sh.Lmax() <= 32) rc = plane_fwd_launch<ST>(f, st, &li);
+        // rows that are not 16-byte aligned: lines of at most 64 positions whose planes fit on chip whole (twice
+        // per SM) go to the whole-plane kernel (378-px config: 0.29 ms against 0.50 ms for the chain kernel; 45x45,
+        // B=64, C=128: 0.30 against 0.41 ms), the rest to the chain kernel
+        if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = plane_fwd_launch<ST>(f, st, &li);
         if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = chain_fwd_launch<ST>(f, st, &li);
         if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = flat_fwd_launch<ST>(f, st, &li);
         if (rc == GSPN_EUNSUPPORTED && a->impl == GSPN_IMPL_AUTO) rc = naive_fwd_launch<ST>(f, st, &li);
