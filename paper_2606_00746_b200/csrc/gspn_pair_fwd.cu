@@ -543,40 +543,38 @@ plane_fwd_kernel(const PairFwdParams p) {
             *reinterpret_cast<uint4*>(yz + o) = make_uint4(0, 0, 0, 0);
     }
     if (threadIdx.x == 0) {
-        for (int s = 0; s < 5; ++s) mbar_init(&bars[s], 33);
+        for (int s = 0; s < 4; ++s) mbar_init(&bars[s], NP);           // one arrival per operand plane
+        mbar_init(&bars[4], NC);
         mbar_init_fence();
     }
     __syncthreads();
 
     const bool act[4] = {p.q[0] >= 0, p.q[1] >= 0, p.q[2] >= 0, p.q[3] >= 0};
     if (warp == NCMP) {
-        // x first (every direction needs it), then the directions in the order the warps consume them
-        for (int t = -1; t < 4; ++t) {
+        // every plane has its own lane (x first: every direction needs it, then the directions in the order the
+        // warps consume them); a lane announces its bytes on the plane's barrier and issues the copy at once, so
+        // all copies of the CTA are in flight after two rounds
+        for (int i = lane; i < NC + 4 * NP; i += 32) {
+            const int t = i < NC ? -1 : (i - NC) / NP, k = i < NC ? i : (i - NC) % NP;
             if (t >= 0 && !act[t]) continue;
-            const int np = t < 0 ? NC : NP;
-            int nbytes = 0;
             unsigned long long a0 = 0;
-            const uint8_t* base = nullptr;
-            uint8_t* dst = nullptr;
-            if (lane < np) {
-                if (t < 0) {
-                    base = (const uint8_t*)p.x;
-                    dst = smem + p.off_x + (size_t)lane * p.xslot;
-                    nbytes = pf_bulk_window(dst, base, (((unsigned long long)b * sh.C + c0 + lane) * HW) * ES, HW * ES,
-                                            p.bytes_x, ES, &a0);
-                } else {
-                    const PfPlane e = pf_plane<NC, ES>(p, p.q[t], b, g, c0, lane);
-                    base = e.base;
-                    dst = smem + p.off_pl + (size_t)(t * NP + lane) * p.plslot;
-                    nbytes = pf_bulk_window(dst, base, e.b0, HW * ES, e.tbytes, ES, &a0);
-                }
+            const uint8_t* base;
+            uint8_t* dst;
+            int nbytes;
+            if (t < 0) {
+                base = (const uint8_t*)p.x;
+                dst = smem + p.off_x + (size_t)k * p.xslot;
+                nbytes = pf_bulk_window(dst, base, (((unsigned long long)b * sh.C + c0 + k) * HW) * ES, HW * ES,
+                                        p.bytes_x, ES, &a0);
+            } else {
+                const PfPlane e = pf_plane<NC, ES>(p, p.q[t], b, g, c0, k);
+                base = e.base;
+                dst = smem + p.off_pl + (size_t)(t * NP + k) * p.plslot;
+                nbytes = pf_bulk_window(dst, base, e.b0, HW * ES, e.tbytes, ES, &a0);
             }
             uint64_t* fb = &bars[t < 0 ? 4 : t];
-            const int total = warp_sum(nbytes);
-            if (lane == 0) mbar_arrive_expect_tx(fb, (uint32_t)total);
-            __syncwarp();
+            mbar_arrive_expect_tx(fb, (uint32_t)nbytes);             // also publishes the tail bytes written above
             if (nbytes > 0) bulk_load_1d(dst, base + a0, (uint32_t)nbytes, fb);
-            mbar_arrive(fb);
         }
     } else {
         uint32_t pf = 0;

@@ -211,40 +211,37 @@ plane_bwd_kernel(const PlaneBwdParams p) {
             *reinterpret_cast<uint4*>(z + o) = make_uint4(0, 0, 0, 0);
     }
     if (threadIdx.x == 0) {
-        for (int s = 0; s < 5; ++s) mbar_init(&bars[s], 33);
+        for (int s = 0; s < 4; ++s) mbar_init(&bars[s], NP);           // one arrival per operand plane
+        mbar_init(&bars[4], 2 * NC);
         mbar_init_fence();
     }
     __syncthreads();
 
     const bool act[4] = {p.q[0] >= 0, p.q[1] >= 0, p.q[2] >= 0, p.q[3] >= 0};
     if (warp == 4) {
-        // x and dy first (every direction needs them), then the directions
-        for (int t = -1; t < 4; ++t) {
+        // every plane has its own lane (x and dy first: every direction needs them); a lane announces its bytes on
+        // the plane's barrier and issues the copy at once
+        for (int i = lane; i < 2 * NC + 4 * NP; i += 32) {
+            const int t = i < 2 * NC ? -1 : (i - 2 * NC) / NP, k = i < 2 * NC ? i : (i - 2 * NC) % NP;
             if (t >= 0 && !act[t]) continue;
-            const int np = t < 0 ? 2 * NC : NP;
-            int nbytes = 0;
             unsigned long long a0 = 0;
-            const uint8_t* base = nullptr;
-            uint8_t* dst = nullptr;
-            if (lane < np) {
-                if (t < 0) {
-                    const int c = lane % NC;
-                    base = (const uint8_t*)(lane < NC ? p.x : p.dy);
-                    dst = smem + (lane < NC ? p.off_x : p.off_dy) + (size_t)c * p.plslot;
-                    nbytes = pb_window(dst, base, (((unsigned long long)b * sh.C + c0 + c) * HW) * ES, HW * ES, p.bytes_x, ES, &a0);
-                } else {
-                    const PbPlane e = pb_plane<NC, ES>(p, p.q[t], b, g, lane);
-                    base = e.base;
-                    dst = smem + p.off_pl + (size_t)(t * NP + lane) * p.plslot;
-                    nbytes = pb_window(dst, base, e.b0, HW * ES, e.tbytes, ES, &a0);
-                }
+            const uint8_t* base;
+            uint8_t* dst;
+            int nbytes;
+            if (t < 0) {
+                const int c = k % NC;
+                base = (const uint8_t*)(k < NC ? p.x : p.dy);
+                dst = smem + (k < NC ? p.off_x : p.off_dy) + (size_t)c * p.plslot;
+                nbytes = pb_window(dst, base, (((unsigned long long)b * sh.C + c0 + c) * HW) * ES, HW * ES, p.bytes_x, ES, &a0);
+            } else {
+                const PbPlane e = pb_plane<NC, ES>(p, p.q[t], b, g, k);
+                base = e.base;
+                dst = smem + p.off_pl + (size_t)(t * NP + k) * p.plslot;
+                nbytes = pb_window(dst, base, e.b0, HW * ES, e.tbytes, ES, &a0);
             }
             uint64_t* fb = &bars[t < 0 ? 4 : t];
-            const int total = warp_sum(nbytes);
-            if (lane == 0) mbar_arrive_expect_tx(fb, (uint32_t)total);
-            __syncwarp();
+            mbar_arrive_expect_tx(fb, (uint32_t)nbytes);             // also publishes the tail bytes written above
             if (nbytes > 0) bulk_load_1d(dst, base + a0, (uint32_t)nbytes, fb);
-            mbar_arrive(fb);
         }
     } else {
         if (warp == 0 && act[0]) plane_bwd_dir<ST, NC, false, false>(p, smem, 0, b, g, lane, act[1]);
