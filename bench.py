@@ -405,8 +405,8 @@ def main():
                 if name == cfg.name and dt == dtype:
                     continue
                 so = 4 if dt == "f32" else 2
-                # the backward of the other configs is timed where the fused chain kernel holds the unit on chip
-                # (C/G <= 4 and the fp32 dx planes of a unit within shared memory): today the 378-px config
+                # the backward of the other configs is timed where a fused single-launch kernel holds the unit on chip
+                # (C/G <= 4 and the fp32 dx planes of a unit within shared memory): the tiny and the 378-px configs
                 ob = impl == gspn.IMPL_AUTO and oc.C // oc.G <= 4 and (oc.C // oc.G) * oc.H * oc.W * 4 <= 100 * 1024
                 r, tt, yy, gg = time_config(gspn, torch, oc, dt, max(5, min(steps, 20)), 3, 1, impl, ob)
                 if ob:

@@ -264,9 +264,12 @@ def test_auto_selects_fused_kernels_where_supported():
     r = pu.check_fwd(cfg, "bf16")
     assert r["ok"] and r["variant"] == "chain_fwd", r
     # 378-px kind of shape (27x27, rows not 16-byte aligned, lines of one warp): the whole-plane kernel
-    cfg = gi.small_config("sel27", 2, 8, 27, 27, 2, seed=10)
+    cfg = gi.small_config("sel27", 2, 8, 27, 27, 2, seed=10, backward=True)
     r = pu.check_fwd(cfg, "bf16")
     assert r["ok"] and r["variant"] == "plane_fwd", r
+    r = pu.check_bwd(cfg, "bf16")
+    assert r["ok"] and r["variant"] == "plane_bwd", r
+    assert gspn.gspn_last_launch_count() == 1
 
 
 def test_chain_kernels_random_shapes():
