@@ -121,6 +121,7 @@ __device__ __forceinline__ void plane_bwd_dir(const PlaneBwdParams& p, uint8_t* 
             h[c] = ld_f(reinterpret_cast<const ST*>(p.h0) + (((size_t)qd * sh.B + b) * sh.C + c0 + c) * Lmax + lane);
         sts32(HS + c * hsc, h[c]);
     }
+#pragma unroll 2
     for (int s = 0; s < Ls; ++s) {
         const uint32_t lo = (uint32_t)(REV ? Ls - 1 - s : s) * step;
         const float w0 = maskf(E::f(E::lds(A[0] + lo)), m_first);       // out-of-grid taps are never used
@@ -148,6 +149,7 @@ __device__ __forceinline__ void plane_bwd_dir(const PlaneBwdParams& p, uint8_t* 
     float carry[NC];
 #pragma unroll
     for (int c = 0; c < NC; ++c) carry[c] = 0.f;
+#pragma unroll 2
     for (int s = Ls - 1; s >= 0; --s) {
         const int li = REV ? Ls - 1 - s : s;                             // image line of this step
         // REV walks the lines upwards in pass 2, !REV downwards: the downward warp waits before line `mid`
