@@ -72,7 +72,8 @@ enum { GSPN_IMPL_AUTO = 0, GSPN_IMPL_NAIVE = 1, GSPN_IMPL_FUSED = 2 /* 16-byte-a
        GSPN_IMPL_FLAT = 3 /* any-shape fused kernel */,
        GSPN_IMPL_CHAIN = 4 /* warp-per-chain kernels (gspn_chain_*.cu) */,
        GSPN_IMPL_PAIR = 5 /* forward: warp per direction carrying all channels of a CTA (gspn_pair_fwd.cu) */,
-       GSPN_IMPL_PLANE = 6 /* forward, small planes: the same with whole operand planes on chip, 4 directions at once */ };
+       GSPN_IMPL_PLANE = 6 /* small planes, forward and backward: whole operand planes on chip, 4 directions at once
+                              (gspn_pair_fwd.cu plane_fwd, gspn_plane_bwd.cu) */ };
 
 /*
  * Forward scan, Eq. (1),(2),(5),(9): the whole
