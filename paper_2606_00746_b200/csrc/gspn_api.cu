@@ -99,7 +99,7 @@ static int bwd_typed(const gspn_args_t* a) {
         rc = plane_bwd_launch<ST>(f, st, &li);
     } else {
         // lines of at most one warp (378-px config: 27x27): the whole-plane kernel where the unit's planes fit on chip
-        // (cfg3 0.96 ms), else the group kernel (2.45 ms; the per-block hand-shakes of the chain kernel cost more
+        // (cfg3 0.89 ms), else the group kernel (2.45 ms; the per-block hand-shakes of the chain kernel cost more
         // there: 2.97 ms); longer lines: the chain kernel
         const bool small = f.sh.Lmax() <= 32;
         rc = small ? plane_bwd_launch<ST>(f, st, &li) : chain_bwd_launch<ST>(f, st, &li);

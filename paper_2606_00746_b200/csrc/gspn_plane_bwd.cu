@@ -68,7 +68,10 @@ __device__ __forceinline__ int pb_window(uint8_t* dst, const uint8_t* base, unsi
 
 // One direction, all NC channels of the unit, on one warp.  VH = false: T->B / B->T (lanes own columns), true:
 // L->R / R->L (lanes own rows); REV = the direction walks the image lines downwards.
-template <typename ST, int NC, bool VH, bool REV>
+// PART 0: the warp does everything.  PART 1 / 2 (NC >= 2): pass 1 is split between the direction's main warp
+// (channels [0, NC/2)) and a helper warp (channels [NC/2, NC)); they meet at a named barrier, then the main warp
+// runs pass 2 for all channels (dw3 is a sum over the group's channels: one warp, fixed order).
+template <typename ST, int NC, bool VH, bool REV, int PART = 0>
 __device__ __forceinline__ void plane_bwd_dir(const PlaneBwdParams& p, uint8_t* smem, const int d, const int b,
                                               const int g, const int lane, const bool pair_sync) {
     using E = Elem<ST>;
@@ -113,9 +116,10 @@ __device__ __forceinline__ void plane_bwd_dir(const PlaneBwdParams& p, uint8_t* 
     mbar_wait(&bars[d], 0);                                       // this direction's planes
 
     // ---------------- pass 1: h in scan order ------------------------------------------------------------
+    constexpr int C0 = PART == 2 ? NC / 2 : 0, C1 = PART == 1 ? NC / 2 : NC;      // this warp's channels in pass 1
     float h[NC];
 #pragma unroll
-    for (int c = 0; c < NC; ++c) {
+    for (int c = C0; c < C1; ++c) {
         h[c] = 0.f;
         if (p.h0 && ok)
             h[c] = ld_f(reinterpret_cast<const ST*>(p.h0) + (((size_t)qd * sh.B + b) * sh.C + c0 + c) * Lmax + lane);
@@ -129,9 +133,9 @@ __device__ __forceinline__ void plane_bwd_dir(const PlaneBwdParams& p, uint8_t* 
         const float w2 = maskf(E::f(E::lds(A[2] + lo)), m_last);
         raw_t lr[NC], xr[NC];
 #pragma unroll
-        for (int c = 0; c < NC; ++c) { lr[c] = E::lds(A[3 + c] + lo); xr[c] = E::lds(AX[c] + lo); }
+        for (int c = C0; c < C1; ++c) { lr[c] = E::lds(A[3 + c] + lo); xr[c] = E::lds(AX[c] + lo); }
 #pragma unroll
-        for (int c = 0; c < NC; ++c) {
+        for (int c = C0; c < C1; ++c) {
             const float hl = __shfl_up_sync(FULLM, h[c], 1), hr = __shfl_down_sync(FULLM, h[c], 1);
             float acc = w1 * h[c];
             acc = fmaf(w0, hl, acc);
@@ -142,6 +146,10 @@ __device__ __forceinline__ void plane_bwd_dir(const PlaneBwdParams& p, uint8_t* 
         }
     }
     __syncwarp();
+    if constexpr (PART != 0) {
+        asm volatile("bar.sync %0, 64;" ::"r"(3 + d) : "memory");      // both halves of h are in shared memory
+        if constexpr (PART == 2) return;
+    }
 
     // ---------------- pass 2: adjoint chain in reverse order ---------------------------------------------
     const bool w_du = p.du != nullptr, w_dl = p.dlam != nullptr, w_dw = p.dw3 != nullptr, w_dx = p.dx != nullptr;
@@ -194,9 +202,11 @@ __device__ __forceinline__ void plane_bwd_dir(const PlaneBwdParams& p, uint8_t* 
 
 // ---------------------------------------------------------------------------------------------------
 template <typename ST, int NC>
-__global__ void __launch_bounds__(160)
+__global__ void __launch_bounds__(NC >= 2 ? 288 : 160)
 plane_bwd_kernel(const PlaneBwdParams p) {
     constexpr int ES = sizeof(ST), NP = 3 + 2 * NC;
+    constexpr bool HELP = NC >= 2;                                // helper warps 4..7 take half of pass 1
+    constexpr int PW = HELP ? 8 : 4, NWARP = PW + 1;              // producer warp, warps of the CTA
     extern __shared__ __align__(1024) uint8_t smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem);           // [0..3] direction planes, [4] x and dy
     const Shape sh = p.sh;
@@ -220,7 +230,7 @@ plane_bwd_kernel(const PlaneBwdParams p) {
     __syncthreads();
 
     const bool act[4] = {p.q[0] >= 0, p.q[1] >= 0, p.q[2] >= 0, p.q[3] >= 0};
-    if (warp == 4) {
+    if (warp == PW) {
         // every plane has its own lane (x and dy first: every direction needs them); a lane announces its bytes on
         // the plane's barrier and issues the copy at once
         for (int i = lane; i < 2 * NC + 4 * NP; i += 32) {
@@ -246,10 +256,17 @@ plane_bwd_kernel(const PlaneBwdParams p) {
             if (nbytes > 0) bulk_load_1d(dst, base + a0, (uint32_t)nbytes, fb);
         }
     } else {
-        if (warp == 0 && act[0]) plane_bwd_dir<ST, NC, false, false>(p, smem, 0, b, g, lane, act[1]);
-        if (warp == 1 && act[1]) plane_bwd_dir<ST, NC, false, true>(p, smem, 1, b, g, lane, act[0]);
-        if (warp == 2 && act[2]) plane_bwd_dir<ST, NC, true, false>(p, smem, 2, b, g, lane, act[3]);
-        if (warp == 3 && act[3]) plane_bwd_dir<ST, NC, true, true>(p, smem, 3, b, g, lane, act[2]);
+        constexpr int PM = HELP ? 1 : 0;
+        if (warp == 0 && act[0]) plane_bwd_dir<ST, NC, false, false, PM>(p, smem, 0, b, g, lane, act[1]);
+        if (warp == 1 && act[1]) plane_bwd_dir<ST, NC, false, true, PM>(p, smem, 1, b, g, lane, act[0]);
+        if (warp == 2 && act[2]) plane_bwd_dir<ST, NC, true, false, PM>(p, smem, 2, b, g, lane, act[3]);
+        if (warp == 3 && act[3]) plane_bwd_dir<ST, NC, true, true, PM>(p, smem, 3, b, g, lane, act[2]);
+        if constexpr (HELP) {
+            if (warp == 4 && act[0]) plane_bwd_dir<ST, NC, false, false, 2>(p, smem, 0, b, g, lane, act[1]);
+            if (warp == 5 && act[1]) plane_bwd_dir<ST, NC, false, true, 2>(p, smem, 1, b, g, lane, act[0]);
+            if (warp == 6 && act[2]) plane_bwd_dir<ST, NC, true, false, 2>(p, smem, 2, b, g, lane, act[3]);
+            if (warp == 7 && act[3]) plane_bwd_dir<ST, NC, true, true, 2>(p, smem, 3, b, g, lane, act[2]);
+        }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // the in-place outputs, before the bulk stores read them
     }
     __syncthreads();
@@ -261,9 +278,9 @@ plane_bwd_kernel(const PlaneBwdParams p) {
         const float* dh = reinterpret_cast<const float*>(smem + p.off_dxh);
         ST* dxg = reinterpret_cast<ST*>(p.dx) + ((size_t)b * sh.C + c0) * HW;
         if (p.Wp == W) {
-            for (int idx = threadIdx.x; idx < NC * hw; idx += 160) st_f(dxg + idx, dv[idx] + dh[idx]);
+            for (int idx = threadIdx.x; idx < NC * hw; idx += 32 * NWARP) st_f(dxg + idx, dv[idx] + dh[idx]);
         } else {
-            for (int ci = warp; ci < NC * H; ci += 5)
+            for (int ci = warp; ci < NC * H; ci += NWARP)
                 for (int j = lane; j < W; j += 32)
                     st_f(dxg + (size_t)ci * W + j, dv[(size_t)ci * p.Wp + j] + dh[(size_t)ci * p.Wp + j]);
         }
@@ -271,7 +288,7 @@ plane_bwd_kernel(const PlaneBwdParams p) {
     // du / dlambda / dw3 lie where u / lambda / the taps lay, at the byte phase they have in HBM (same tensor
     // offsets): the 16-byte-aligned interior of a plane leaves by ONE bulk store, the few elements before and
     // after it by ordinary stores
-    for (int pl = warp; pl < 4 * NP; pl += 5) {
+    for (int pl = warp; pl < 4 * NP; pl += NWARP) {
         const int d = pl / NP, k = pl % NP;
         if (!act[d]) continue;
         ST* out = k < 3 ? reinterpret_cast<ST*>(p.dw3) : (k < 3 + NC ? reinterpret_cast<ST*>(p.dlam) : reinterpret_cast<ST*>(p.du));
@@ -323,7 +340,7 @@ static int launch_plane_bwd(const PlaneBwdParams& prm, int items, cudaStream_t s
     auto kern = plane_bwd_kernel<ST, NC>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prm.total);
     if (e != cudaSuccess) { set_error("plane bwd: cudaFuncSetAttribute(%u B): %s", prm.total, cudaGetErrorString(e)); return GSPN_ECUDA; }
-    kern<<<items, 160, prm.total, st>>>(prm);
+    kern<<<items, NC >= 2 ? 288 : 160, prm.total, st>>>(prm);
     e = cudaGetLastError();
     if (e != cudaSuccess) { set_error("plane bwd: launch failed: %s", cudaGetErrorString(e)); return GSPN_ECUDA; }
     return GSPN_OK;
