@@ -5,6 +5,7 @@ closed form, a library routine (numpy cumsum / matmul / polynomial, scipy lfilte
 a dense-matrix brute force of Eq. (4), an invariant or a
 finite difference.  Runs on CPU only.
 """
+import math
 import os
 
 import numpy as np
@@ -593,3 +594,57 @@ def test_normalized_taps_feed_the_scan_stably():
         Ls = H if q < 2 else W
         bound = lam[q].max() * Ls
         assert np.all(np.abs(h[q]) <= bound + 1e-12)
+
+
+def test_normalize_bwd_magnitude_closed_form_and_dominance():
+    """Magnitude mode of the Eq. (3) adjoint (the scale A of the normalize_bwd gate, tests/parity_util.py).
+    Closed form at an interior pixel with equal logits a and dw = (1, 0, 0): s = sigmoid(a), S = 3s, w_k = 1/3, so
+    the plain adjoint is (1-s)*(1 - 1/3)/3 = (1-s)*2/9 for k = 0 and -(1-s)/9 for k = 1, 2, while the sum of the
+    absolute values of the same terms is (1-s)*(1 + 1/3)/3 = (1-s)*4/9 and (1-s)/9."""
+    for a in (-1.5, 0.0, 0.7):
+        wt = np.full((1, 1, 1, 3, 3, 3), a)
+        dw = np.zeros_like(wt)
+        dw[0, 0, 0, 0, 1, 1] = 1.0
+        s = 1.0 / (1.0 + math.exp(-a))
+        g = orc.normalize_bwd(wt, dw, 1)[0, 0, 0, :, 1, 1]
+        m = orc.normalize_bwd(wt, dw, 1, magnitude=True)[0, 0, 0, :, 1, 1]
+        np.testing.assert_allclose(g, [(1 - s) * 2 / 9, -(1 - s) / 9, -(1 - s) / 9], rtol=1e-13)
+        np.testing.assert_allclose(m, [(1 - s) * 4 / 9, (1 - s) / 9, (1 - s) / 9], rtol=1e-13)
+    rng = np.random.default_rng(41)
+    wt = rng.normal(0, 2, (4, 2, 2, 3, 5, 6))
+    dw = rng.standard_normal(wt.shape)
+    g = orc.normalize_bwd(wt, dw, 15)
+    m = orc.normalize_bwd(wt, dw, 15, magnitude=True)
+    assert np.all(m >= np.abs(g) - 1e-15) and np.all(m >= 0)
+    # the sign of dw does not matter to the magnitude; it is linear under positive scaling
+    np.testing.assert_allclose(orc.normalize_bwd(wt, -dw, 15, magnitude=True), m, rtol=1e-14)
+    np.testing.assert_allclose(orc.normalize_bwd(wt, 2.5 * dw, 15, magnitude=True), 2.5 * m, rtol=1e-13)
+    # one nonzero tap gradient per pixel: the in-bracket terms dw_k and -dw_k w_k have opposite signs for tap k (so the
+    # magnitude is |dw_k|(1 + w_k) against |dw_k|(1 - w_k)) and a single term for the other taps (magnitude = |value|)
+    one = np.zeros_like(dw)
+    one[:, :, :, 1] = dw[:, :, :, 1]
+    g1 = orc.normalize_bwd(wt, one, 15)
+    m1 = orc.normalize_bwd(wt, one, 15, magnitude=True)
+    w = orc.normalize(wt, 15)
+    np.testing.assert_allclose(m1[:, :, :, 0], np.abs(g1[:, :, :, 0]), rtol=1e-12, atol=1e-300)
+    np.testing.assert_allclose(m1[:, :, :, 2], np.abs(g1[:, :, :, 2]), rtol=1e-12, atol=1e-300)
+    np.testing.assert_allclose(m1[:, :, :, 1] * (1 - w[:, :, :, 1]), np.abs(g1[:, :, :, 1]) * (1 + w[:, :, :, 1]),
+                               rtol=1e-10, atol=1e-300)
+
+
+def test_float_build_of_backward_tracks_double_build():
+    """The pinned-order float build of the adjoint (the timed cpu_baseline) stays within 1e-5 of the magnitude
+    scale of the double build on every gradient."""
+    rng = np.random.default_rng(42)
+    B, C, H, W, G = 2, 8, 31, 26, 2
+    x, w3, lam, u = rand_problem(rng, B, C, H, W, G, 15)
+    dy = rng.standard_normal(x.shape)
+    h0 = rng.standard_normal((4, B, C, max(H, W)))
+    s = [a.astype(np.float32) for a in (x, w3, lam, u, dy, h0)]
+    d = [a.astype(np.float64) for a in s]
+    g64 = orc.bwd(d[0], d[1], d[2], d[3], d[4], G, 15, h0=d[5])
+    A = orc.bwd_magnitude(d[0], d[1], d[2], d[3], d[4], G, 15, h0=d[5])
+    g32 = orc.bwd(s[0], s[1], s[2], s[3], s[4], G, 15, h0=s[5])
+    for k in ("dx", "dlambda", "du", "dw3", "dh0"):
+        assert g32[k].dtype == np.float32
+        assert np.all(np.abs(g32[k] - g64[k]) <= np.maximum(1e-5 * A[k], 1e-6)), k
