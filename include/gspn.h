@@ -73,7 +73,9 @@ enum { GSPN_IMPL_AUTO = 0, GSPN_IMPL_NAIVE = 1, GSPN_IMPL_FUSED = 2 /* 16-byte-a
        GSPN_IMPL_CHAIN = 4 /* warp-per-chain kernels (gspn_chain_*.cu) */,
        GSPN_IMPL_PAIR = 5 /* forward: warp per direction carrying all channels of a CTA (gspn_pair_fwd.cu) */,
        GSPN_IMPL_PLANE = 6 /* small planes, forward and backward: whole operand planes on chip, 4 directions at once
-                              (gspn_pair_fwd.cu plane_fwd, gspn_plane_bwd.cu) */ };
+                              (gspn_pair_fwd.cu plane_fwd, gspn_plane_bwd.cu) */,
+       GSPN_IMPL_LINE = 7 /* 16-byte-aligned rows: warp per (channel, direction) line, several positions per lane,
+                              one fp32 accumulator plane per channel (gspn_line_fwd.cu, gspn_line_bwd.cu) */ };
 
 /*
  * Forward scan, Eq. (1),(2),(5),(9): the whole

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libgspn.so")
 
 DIR_TB, DIR_BT, DIR_LR, DIR_RL, DIR_ALL = 1, 2, 4, 8, 15
 F32, BF16 = 0, 1
-IMPL_AUTO, IMPL_NAIVE, IMPL_FUSED, IMPL_FLAT, IMPL_CHAIN, IMPL_PAIR, IMPL_PLANE = 0, 1, 2, 3, 4, 5, 6
+IMPL_AUTO, IMPL_NAIVE, IMPL_FUSED, IMPL_FLAT, IMPL_CHAIN, IMPL_PAIR, IMPL_PLANE, IMPL_LINE = 0, 1, 2, 3, 4, 5, 6, 7
 STATUS = {0: "GSPN_OK", 1: "GSPN_EINVAL", 2: "GSPN_EUNSUPPORTED", 3: "GSPN_EALIGN",
           4: "GSPN_EWORKSPACE", 5: "GSPN_ECUDA"}
 

@@ -64,8 +64,11 @@ static int fwd_typed(const gspn_args_t* a) {
         rc = pair_fwd_launch<ST>(f, st, &li);
     } else if (a->impl == GSPN_IMPL_PLANE) {
         rc = plane_fwd_launch<ST>(f, st, &li);
+    } else if (a->impl == GSPN_IMPL_LINE) {
+        rc = line_fwd_launch<ST>(f, st, &li);
     } else {
-        rc = fused_fwd_launch<ST>(f, st, &li);
+        rc = a->impl == GSPN_IMPL_AUTO ? line_fwd_launch<ST>(f, st, &li) : GSPN_EUNSUPPORTED;
+        if (rc == GSPN_EUNSUPPORTED) rc = fused_fwd_launch<ST>(f, st, &li);
         // rows that are not 16-byte aligned: lines of at most 64 positions whose planes fit on chip whole (twice
         // per SM) go to the whole-plane kernel (378-px config: 0.29 ms against 0.50 ms for the chain kernel; 45x45,
         // B=64, C=128: 0.30 against 0.41 ms), the rest to the chain kernel
@@ -117,7 +120,7 @@ static int check_ex(const gspn_args_t* a) {
         set_error("gspn_args_t.struct_size=%zu, expected %zu", a->struct_size, sizeof(gspn_args_t));
         return GSPN_EINVAL;
     }
-    if (a->impl < GSPN_IMPL_AUTO || a->impl > GSPN_IMPL_PLANE) {
+    if (a->impl < GSPN_IMPL_AUTO || a->impl > GSPN_IMPL_LINE) {
         set_error("unknown impl %d", a->impl);
         return GSPN_EINVAL;
     }

@@ -34,6 +34,10 @@ template <typename ST> int plane_fwd_launch(const FwdArgs<ST>& a, cudaStream_t s
 // whole-plane backward for small planes (gspn_plane_bwd.cu): lines of at most one warp, C/G in {1, 2, 4}
 template <typename ST> int plane_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 
+// line kernels (gspn_line_fwd.cu / gspn_line_bwd.cu): 16-byte-aligned rows, warp per (channel, direction) line with 1, 2 or
+// 4 positions per lane, NC channels of a unit per CTA sharing the taps, one fp32 accumulator plane per channel.
+template <typename ST> int line_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
+
 // merge (gspn_merge.cu)
 template <typename ST>
 int merge_launch(const ST* y_dirs, const float* m, ST* y, int D, int B, int C, int H, int W,

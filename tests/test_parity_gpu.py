@@ -16,15 +16,16 @@ pytestmark = pytest.mark.gpu
 
 IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO]
 IMPL_IDS = ["naive", "auto"]
-FWD_IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO, gspn.IMPL_FLAT, gspn.IMPL_CHAIN, gspn.IMPL_PAIR, gspn.IMPL_PLANE]
-FWD_IMPL_IDS = ["naive", "auto", "flat", "chain", "pair", "plane"]
+FWD_IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO, gspn.IMPL_FLAT, gspn.IMPL_CHAIN, gspn.IMPL_PAIR, gspn.IMPL_PLANE, gspn.IMPL_LINE]
+FWD_IMPL_IDS = ["naive", "auto", "flat", "chain", "pair", "plane", "line"]
 
 # (B, C, H, W, G): degenerate lines, W in {1,2,3}, H != W, beyond one warp, ragged tails, cg in {1,C}
 SMALL_SHAPES = [
     (1, 1, 1, 1, 1), (1, 2, 1, 5, 1), (1, 2, 5, 1, 2), (2, 4, 4, 2, 2), (1, 3, 3, 3, 1),
     (2, 4, 5, 7, 2), (2, 4, 7, 5, 4), (1, 8, 16, 16, 8), (1, 4, 33, 35, 1), (2, 6, 40, 24, 3),
     (1, 4, 27, 27, 1), (1, 2, 73, 73, 2), (1, 8, 56, 56, 1), (1, 2, 128, 128, 1), (1, 2, 64, 130, 2),
-    (1, 2, 100, 36, 1),
+    (1, 2, 100, 36, 1), (2, 8, 24, 40, 2), (1, 4, 8, 128, 1), (1, 4, 128, 8, 2), (2, 4, 12, 16, 4), (1, 4, 20, 12, 2),
+    (1, 8, 60, 56, 1), (1, 4, 4, 4, 4), (1, 8, 128, 120, 2),
 ]
 
 
@@ -32,12 +33,22 @@ def _ids(shapes):
     return ["x".join(map(str, s)) for s in shapes]
 
 
+def _unsupported_is_none(impl, fn):
+    """As _fwd_or_skip inside a loop over shapes: None for a shape the forced kernel does not hold."""
+    try:
+        return fn()
+    except gspn.GspnError as ex:
+        if impl in (gspn.IMPL_PAIR, gspn.IMPL_PLANE, gspn.IMPL_LINE) and ex.status == 2:
+            return None
+        raise
+
+
 def _fwd_or_skip(impl, fn):
     """The pair / plane kernels keep whole fp32 planes on chip: shapes they report as unsupported are skipped."""
     try:
         return fn()
     except gspn.GspnError as ex:
-        if impl in (gspn.IMPL_PAIR, gspn.IMPL_PLANE) and ex.status == 2:          # GSPN_EUNSUPPORTED
+        if impl in (gspn.IMPL_PAIR, gspn.IMPL_PLANE, gspn.IMPL_LINE) and ex.status == 2:          # GSPN_EUNSUPPORTED
             pytest.skip(str(ex))
         raise
 
@@ -56,19 +67,28 @@ def test_fwd_small_shapes(shape, dtype, impl):
 @pytest.mark.parametrize("impl", FWD_IMPLS, ids=FWD_IMPL_IDS)
 @pytest.mark.parametrize("mask", [1, 2, 4, 8, 3, 12, 5, 10, 7, 14])
 def test_fwd_direction_masks(mask, impl):
-    for dtype in ("f32", "bf16"):
-        cfg = gi.small_config("m", 2, 4, 9, 12, 2, dir_mask=mask, seed=5 + mask)
-        r = pu.check_fwd(cfg, dtype, impl=impl)
-        assert r["ok"], (dtype, r)
+    ran = 0
+    for shape in [(2, 4, 9, 12, 2), (2, 4, 8, 16, 2), (1, 2, 40, 64, 1)]:
+        for dtype in ("f32", "bf16"):
+            cfg = gi.small_config("m", *shape, dir_mask=mask, seed=5 + mask)
+            r = _unsupported_is_none(impl, lambda: pu.check_fwd(cfg, dtype, impl=impl))
+            if r is not None:
+                ran += 1
+                assert r["ok"], (shape, dtype, r)
+    assert ran >= 2
 
 
 @pytest.mark.parametrize("impl", FWD_IMPLS, ids=FWD_IMPL_IDS)
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
 def test_fwd_with_initial_state(dtype, impl):
-    for shape in [(2, 4, 6, 9, 2), (1, 2, 20, 40, 1)]:
+    ran = 0
+    for shape in [(2, 4, 6, 9, 2), (1, 2, 20, 40, 1), (2, 4, 16, 8, 2), (1, 4, 128, 64, 4)]:
         cfg = gi.small_config("h0", *shape, seed=21)
-        r = pu.check_fwd(cfg, dtype, impl=impl, with_h0=True)
-        assert r["ok"], r
+        r = _unsupported_is_none(impl, lambda: pu.check_fwd(cfg, dtype, impl=impl, with_h0=True))
+        if r is not None:
+            ran += 1
+            assert r["ok"], (shape, r)
+    assert ran >= 2
 
 
 @pytest.mark.parametrize("impl", FWD_IMPLS, ids=FWD_IMPL_IDS)
