@@ -153,7 +153,7 @@ template <int N> __device__ __forceinline__ void stf(float* p, const float (&f)[
 // Encodes a tiled, unswizzled tensor map over `rank` dimensions (dims[0] is the contiguous one,
 // strides_bytes[i] is the stride of dims[i+1]).  Returns false and sets the library error on failure.
 bool encode_tensor_map(CUtensorMap* out, int es, void* base, int rank, const uint64_t* dims,
-                       const uint64_t* strides_bytes, const uint32_t* box);
+                       const uint64_t* strides_bytes, const uint32_t* box, int swizzle32 = 0);
 
 static inline int round_up_int(int v, int m) { return (v + m - 1) / m * m; }
 

@@ -51,6 +51,19 @@ template <typename ST> __device__ __forceinline__ float line_elem(const uint32_t
     else return (e & 1) ? __uint_as_float(w[e >> 1] & 0xffff0000u) : __uint_as_float(w[e >> 1] << 16);
 }
 
+// spinning wait (mbarrier.test_wait never suspends the thread)
+__device__ __forceinline__ void mbar_wait_spin(uint64_t* b, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "GSPN_SPIN:\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra GSPN_SPIN_DONE;\n"
+        "bra GSPN_SPIN;\n"
+        "GSPN_SPIN_DONE:\n"
+        "}\n" ::"r"(smem_u32(b)), "r"(parity) : "memory");
+}
+
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
