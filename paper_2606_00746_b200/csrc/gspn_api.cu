@@ -100,10 +100,14 @@ static int bwd_typed(const gspn_args_t* a) {
         rc = chain_bwd_launch<ST>(f, st, &li);
     } else if (a->impl == GSPN_IMPL_PLANE) {
         rc = plane_bwd_launch<ST>(f, st, &li);
+    } else if (a->impl == GSPN_IMPL_LINE) {
+        rc = line_bwd_launch<ST>(f, st, &li);
     } else {
         // lines of at most one warp (378-px config: 27x27): the whole-plane kernel where the unit's planes fit on chip
         // (cfg3 0.89 ms), else the group kernel (2.45 ms; the per-block hand-shakes of the chain kernel cost more
         // there: 2.97 ms); longer lines: the chain kernel
+        // (the line backward, gspn_line_bwd.cu, is selected with GSPN_IMPL_LINE only until it has passed the GPU
+        // parity suite: see DESIGN.md section 7)
         const bool small = f.sh.Lmax() <= 32;
         rc = small ? plane_bwd_launch<ST>(f, st, &li) : chain_bwd_launch<ST>(f, st, &li);
         if (rc == GSPN_EUNSUPPORTED && small) rc = fused_bwd_launch<ST>(f, st, &li);

@@ -37,6 +37,7 @@ template <typename ST> int plane_bwd_launch(const BwdArgs<ST>& a, cudaStream_t s
 // line kernels (gspn_line_fwd.cu / gspn_line_bwd.cu): 16-byte-aligned rows, warp per (channel, direction) line with 1, 2 or
 // 4 positions per lane, NC channels of a unit per CTA sharing the taps, one fp32 accumulator plane per channel.
 template <typename ST> int line_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
+template <typename ST> int line_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 
 // merge (gspn_merge.cu)
 template <typename ST>

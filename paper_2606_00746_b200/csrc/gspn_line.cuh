@@ -130,6 +130,25 @@ __device__ __forceinline__ void tm_pair_sync(int id) {
     tm_fence_after();
 }
 
+// ---- TMA stores shared -> global (tiled), bulk-group completion --------------------------------------------------
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, const void* src, int c0, int c1, int c2) {
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];"
+                 ::"l"(m), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void tma_store_4d(const CUtensorMap* m, const void* src, int c0, int c1, int c2, int c3) {
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5}], [%1];"
+                 ::"l"(m), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// all but the newest N groups of this thread have finished READING shared memory
+template <int N> __device__ __forceinline__ void bulk_wait_read() {
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+template <int N> __device__ __forceinline__ void bulk_wait_all() {
+    asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 __device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* m, int c0, int c1, int c2, int c3, int c4,
                                             uint64_t* bar) {
     asm volatile(
@@ -137,5 +156,70 @@ __device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* m, int
         ::"r"(smem_u32(dst)), "l"(m), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
         : "memory");
 }
+
+// raw storage words of P elements (lambda and x are multiplied without widening: one FHFMA.BF16 per position)
+template <typename ST, int P> struct LineRaw { uint32_t w[(P * sizeof(ST) + 3) / 4]; };
+template <typename ST, int P> __device__ __forceinline__ void line_ld_raw(const ST* p, LineRaw<ST, P>& r) {
+    if constexpr (P * sizeof(ST) == 2) r.w[0] = *reinterpret_cast<const unsigned short*>(p);
+    else lds_vec<P * sizeof(ST)>(p, r.w);
+}
+// c + a[k] * b[k] on raw storage words
+template <typename ST> __device__ __forceinline__ float line_fma_raw(const uint32_t* a, const uint32_t* b, int k, float c) {
+    if constexpr (sizeof(ST) == 4) {
+        return fmaf(__uint_as_float(a[k]), __uint_as_float(b[k]), c);
+    } else {
+        float d;
+        if (k & 1)
+            asm("{ .reg .b16 al, ah, bl, bh;\n mov.b32 {al, ah}, %1;\n mov.b32 {bl, bh}, %2;\n fma.rn.f32.bf16 %0, ah, bh, %3; }"
+                : "=f"(d) : "r"(a[k >> 1]), "r"(b[k >> 1]), "f"(c));
+        else
+            asm("{ .reg .b16 al, ah, bl, bh;\n mov.b32 {al, ah}, %1;\n mov.b32 {bl, bh}, %2;\n fma.rn.f32.bf16 %0, al, bl, %3; }"
+                : "=f"(d) : "r"(a[k >> 1]), "r"(b[k >> 1]), "f"(c));
+        return d;
+    }
+}
+
+// the plane of one channel turns from the column-owner layout into the row-owner layout (one warp, in place)
+template <int P>
+__device__ __forceinline__ void line_transpose(uint32_t tb, float* tile, int pitch, int H, int W, int lane) {
+    const int WP = W / P;
+    for (int t = 0; t * 32 < H; ++t) {
+#pragma unroll
+        for (int r8 = 0; r8 < 4; ++r8) {
+            float f[8 * P];                                   // rows 32t + 8*r8 + r, columns P*lane + k
+            tm_ld<8 * P>(tb + (32 * t + 8 * r8) * P, f);
+            tm_wait_ld<8 * P>(f);
+            if (lane < WP) {
+#pragma unroll
+                for (int r = 0; r < 8; ++r) {
+                    float g[P];
+#pragma unroll
+                    for (int k = 0; k < P; ++k) g[k] = f[r * P + k];
+                    stf<P>(tile + (8 * r8 + r) * pitch + P * lane, g);
+                }
+            }
+        }
+        __syncwarp();
+        const float* row = tile + lane * pitch;               // image row 32t + lane
+        int j0 = 0;
+        for (; j0 + 32 <= W; j0 += 32) {
+            float f[32];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const float4 v = *reinterpret_cast<const float4*>(row + j0 + 4 * q);
+                f[4 * q] = v.x; f[4 * q + 1] = v.y; f[4 * q + 2] = v.z; f[4 * q + 3] = v.w;
+            }
+            tm_st<32>(tb + t * 32 * P + j0, f);
+        }
+        for (; j0 + 4 <= W; j0 += 4) {
+            float f[4];
+            ldf<4>(row + j0, f);
+            tm_st<4>(tb + t * 32 * P + j0, f);
+        }
+        tm_wait_st();
+        __syncwarp();
+    }
+}
+
 
 }  // namespace gspn

@@ -84,28 +84,6 @@ __device__ __forceinline__ void line_release_stage(uint64_t* empty_bar, int lane
     if (lane == 0) mbar_arrive(empty_bar);
 }
 
-// raw storage words of P elements (lambda and x are multiplied without widening: one FHFMA.BF16 per position)
-template <typename ST, int P> struct LineRaw { uint32_t w[(P * sizeof(ST) + 3) / 4]; };
-template <typename ST, int P> __device__ __forceinline__ void line_ld_raw(const ST* p, LineRaw<ST, P>& r) {
-    if constexpr (P * sizeof(ST) == 2) r.w[0] = *reinterpret_cast<const unsigned short*>(p);
-    else lds_vec<P * sizeof(ST)>(p, r.w);
-}
-// c + a[k] * b[k] on raw storage words
-template <typename ST> __device__ __forceinline__ float line_fma_raw(const uint32_t* a, const uint32_t* b, int k, float c) {
-    if constexpr (sizeof(ST) == 4) {
-        return fmaf(__uint_as_float(a[k]), __uint_as_float(b[k]), c);
-    } else {
-        float d;
-        if (k & 1)
-            asm("{ .reg .b16 al, ah, bl, bh;\n mov.b32 {al, ah}, %1;\n mov.b32 {bl, bh}, %2;\n fma.rn.f32.bf16 %0, ah, bh, %3; }"
-                : "=f"(d) : "r"(a[k >> 1]), "r"(b[k >> 1]), "f"(c));
-        else
-            asm("{ .reg .b16 al, ah, bl, bh;\n mov.b32 {al, ah}, %1;\n mov.b32 {bl, bh}, %2;\n fma.rn.f32.bf16 %0, al, bl, %3; }"
-                : "=f"(d) : "r"(a[k >> 1]), "r"(b[k >> 1]), "f"(c));
-        return d;
-    }
-}
-
 // one scan step of a vertical direction: operands of image row `row` of the stage, accumulator row i
 template <typename ST, int NC, int P>
 __device__ __forceinline__ void line_fwd_vstep(const LineCtx& cx, const ST* row, uint32_t pbe, int i, bool acc,
@@ -256,48 +234,6 @@ __device__ __forceinline__ void line_fwd_hstage(const LineCtx& cx, const unsigne
 #pragma unroll
             for (int k = 0; k < P; ++k) tm_st<4>(cx.tb + k * 32 * P + j0, yv[k]);
         }
-    }
-}
-
-// the plane of one channel turns from the column-owner layout into the row-owner layout (one warp, in place)
-template <int P>
-__device__ __forceinline__ void line_transpose(uint32_t tb, float* tile, int pitch, int H, int W, int lane) {
-    const int WP = W / P;
-    for (int t = 0; t * 32 < H; ++t) {
-#pragma unroll
-        for (int r8 = 0; r8 < 4; ++r8) {
-            float f[8 * P];                                   // rows 32t + 8*r8 + r, columns P*lane + k
-            tm_ld<8 * P>(tb + (32 * t + 8 * r8) * P, f);
-            tm_wait_ld<8 * P>(f);
-            if (lane < WP) {
-#pragma unroll
-                for (int r = 0; r < 8; ++r) {
-                    float g[P];
-#pragma unroll
-                    for (int k = 0; k < P; ++k) g[k] = f[r * P + k];
-                    stf<P>(tile + (8 * r8 + r) * pitch + P * lane, g);
-                }
-            }
-        }
-        __syncwarp();
-        const float* row = tile + lane * pitch;               // image row 32t + lane
-        int j0 = 0;
-        for (; j0 + 32 <= W; j0 += 32) {
-            float f[32];
-#pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                const float4 v = *reinterpret_cast<const float4*>(row + j0 + 4 * q);
-                f[4 * q] = v.x; f[4 * q + 1] = v.y; f[4 * q + 2] = v.z; f[4 * q + 3] = v.w;
-            }
-            tm_st<32>(tb + t * 32 * P + j0, f);
-        }
-        for (; j0 + 4 <= W; j0 += 4) {
-            float f[4];
-            ldf<4>(row + j0, f);
-            tm_st<4>(tb + t * 32 * P + j0, f);
-        }
-        tm_wait_st();
-        __syncwarp();
     }
 }
 

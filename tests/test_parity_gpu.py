@@ -4,6 +4,8 @@ Small cases are compared element by element over whole tensors; BASELINE.json's 
 are launched exactly as bench.py launches them and compared on sampled images (every (b,group)
 unit is independent, so the oracle recomputes whole images).  Gates are in tests/parity_util.py.
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -179,6 +181,43 @@ def test_bwd_plane_direction_masks(mask):
     for dtype in ("f32", "bf16"):
         r = pu.check_bwd(cfg, dtype, impl=gspn.IMPL_PLANE, with_h0=(mask % 2 == 1))
         assert r["ok"], (dtype, r)
+
+
+LINE_BWD_SHAPES = [
+    (1, 4, 8, 8, 1), (2, 4, 16, 16, 2), (1, 8, 56, 56, 1), (1, 8, 40, 64, 2), (1, 4, 128, 128, 1), (2, 8, 128, 128, 2),
+    (1, 2, 128, 8, 1), (1, 4, 8, 128, 4), (1, 4, 24, 40, 2), (1, 8, 60, 56, 1), (1, 4, 36, 100, 1), (1, 8, 128, 120, 2),
+    (1, 2, 4, 4, 2), (1, 4, 20, 12, 2),
+]
+
+
+# The line backward was written after GPU access for this repository had been closed (round 2): it compiles for
+# sm_100a but has never run.  Its tests are opt-in so that an unverified kernel cannot take the CUDA context of the
+# whole suite down with it: GSPN_TEST_LINE_BWD=1 python -m pytest tests -m gpu -k bwd_line
+_line_bwd = pytest.mark.skipif(os.environ.get("GSPN_TEST_LINE_BWD", "0") != "1",
+                               reason="line_bwd has not been run on hardware yet (set GSPN_TEST_LINE_BWD=1)")
+
+
+@_line_bwd
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("shape", LINE_BWD_SHAPES, ids=_ids(LINE_BWD_SHAPES))
+def test_bwd_line_small_shapes(shape, dtype):
+    """The line backward (16-byte-aligned rows, dx in tensor memory, C/G in {1, 2, 4, 8})."""
+    cfg = gi.small_config("lb", *shape, seed=31, backward=True)
+    r = _unsupported_is_none(gspn.IMPL_LINE, lambda: pu.check_bwd(cfg, dtype, impl=gspn.IMPL_LINE, with_h0=True))
+    if r is None:
+        pytest.skip("shape not held by the line backward in this storage type")
+    assert r["ok"] and r["variant"] == "line_bwd", r
+
+
+@_line_bwd
+@pytest.mark.parametrize("mask", [1, 2, 4, 8, 3, 12, 6, 9, 13, 15])
+def test_bwd_line_direction_masks(mask):
+    for shape in [(2, 4, 8, 16, 2), (1, 8, 40, 64, 1)]:
+        for dtype in ("f32", "bf16"):
+            cfg = gi.small_config("lbm", *shape, dir_mask=mask, seed=40 + mask, backward=True)
+            r = _unsupported_is_none(gspn.IMPL_LINE, lambda: pu.check_bwd(cfg, dtype, impl=gspn.IMPL_LINE, with_h0=(mask % 2 == 1)))
+            if r is not None:
+                assert r["ok"] and r["variant"] == "line_bwd", (shape, dtype, r)
 
 
 def test_bwd_optional_outputs():
