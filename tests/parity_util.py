@@ -6,7 +6,7 @@ the SAME (already storage-rounded) inputs, `A` the oracle's magnitude run (sum o
 each output), i.e. the scale rounding errors are relative to:
 
   fp32 : |a-b| <= max(1e-5*A, 1e-6)                                   elementwise
-  bf16 : ||a-b||_2 / ||b||_2 <= 3e-3                                  and, elementwise,
+  bf16 : ||a-b||_2 / ||b||_2 <= 3e-3  (tensors of more than 16 elements)  and, elementwise,
          |a-b| <= 0.5*ulp_bf16(max(|a|,|b|))*(1+2^-6) + 1e-5*max(A,1e-6)
          (the fp32 tolerance plus the one unavoidable storage rounding)
 """
@@ -17,6 +17,9 @@ import torch
 
 import gspn_inputs as gi
 from oracle import gspn_oracle as orc
+
+
+SMALL_L2_ELEMS = 16       # tensors this small are gated elementwise only (bf16)
 
 
 def np64(t: torch.Tensor) -> np.ndarray:
@@ -49,7 +52,9 @@ def gate(a: np.ndarray, b: np.ndarray, A: np.ndarray, dtype: str) -> dict:
         tol = half_ulp_bf16(np.maximum(np.abs(a), np.abs(b))) * (1 + 2.0 ** -6) + 1e-5 * np.maximum(A, 1e-6)
         viol = err > tol
         out["violations"] = int(viol.sum())
-        out["ok"] = out["violations"] == 0 and out["rel_l2"] <= 3e-3
+        # a handful of elements: one storage rounding of 2^-9 relative can exceed 3e-3 of so short a vector, so the
+        # norm-wise gate is reported but only the elementwise gate (which bounds every element) decides there
+        out["ok"] = out["violations"] == 0 and (out["rel_l2"] <= 3e-3 or a.size <= SMALL_L2_ELEMS)
     out["nonfinite"] = int((~np.isfinite(a)).sum())
     out["ok"] = bool(out["ok"] and out["nonfinite"] == 0)
     return out

@@ -1,0 +1,221 @@
+"""Round-2 GPU parity additions ("Parity holes"): the host entry points, every image of the full-size
+configs, the out-of-grid taps (reading 3), run-to-run bit identity, the backward of the aligned benchmark
+shapes through GSPN_IMPL_AUTO with the variant reported, optional outputs per kernel.
+
+Collected after test_parity_gpu.py on purpose: these cases were written while GPU access was closed for this
+repository, so a failure here must not hide the results of the suite that had already run on hardware.
+"""
+import numpy as np
+import pytest
+import torch
+
+import gspn_inputs as gi
+import paper_2606_00746_b200 as gspn
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+
+
+def _try(fn):
+    """None when the forced kernel reports the shape as unsupported."""
+    try:
+        return fn()
+    except gspn.GspnError as ex:
+        if ex.status == 2:
+            return None
+        raise
+
+
+# ---------------------------------------------------------------------------------- host entry points (hole a)
+@pytest.mark.parametrize("pinned", [True, False], ids=["pinned", "pageable"])
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_host_entry_points_match_the_oracle(dtype, pinned):
+    """gspn_scan_fwd_host / gspn_scan_bwd_host (the calls bench.py's e2e leg times) on an odd shape, every output
+    gated against the oracle."""
+    cfg = gi.small_config("host", 2, 4, 37, 41, 2, seed=51, backward=True)
+    t = gi.make_inputs(cfg, dtype, device="cpu", with_dy=True)
+    host = {k: (v.contiguous().pin_memory() if pinned else v.contiguous().clone()) for k, v in t.items()}
+    L = max(cfg.H, cfg.W)
+    st = host["x"].dtype
+    mk = (lambda *s: torch.empty(*s, dtype=st).pin_memory()) if pinned else (lambda *s: torch.empty(*s, dtype=st))
+    y = mk(*host["x"].shape)
+    gspn.gspn_scan_fwd_host(host["x"], host["w3"], host["lam"], host["u"], y, cfg.G, cfg.dir_mask)
+    yo, A = pu.oracle_fwd(t, cfg)
+    r = pu.gate(pu.np64(y), yo, A, dtype)
+    assert r["ok"], r
+    outs = {"dx": mk(*host["x"].shape), "dlambda": mk(*host["lam"].shape), "du": mk(*host["u"].shape),
+            "dw3": mk(*host["w3"].shape), "dh0": mk(cfg.D, cfg.B, cfg.C, L)}
+    gspn.gspn_scan_bwd_host(host["x"], host["w3"], host["lam"], host["u"], host["dy"], outs["dx"], outs["dlambda"],
+                            outs["du"], outs["dw3"], outs["dh0"], cfg.G, cfg.dir_mask)
+    go, Ag = pu.oracle_bwd(t, cfg)
+    for k in ("dx", "dlambda", "du", "dw3", "dh0"):
+        r = pu.gate(pu.np64(outs[k]), go[k], Ag[k], dtype)
+        assert r["ok"], (k, r)
+
+
+# ---------------------------------------------------------------------------------- every image (hole b, c)
+def _all_images_fwd(cfg, dtype, t, y, chunk):
+    for b0 in range(0, cfg.B, chunk):
+        b1 = min(cfg.B, b0 + chunk)
+        sub = gi.with_batch(cfg, b1 - b0)
+        yo, A = pu.oracle_fwd(pu._slice(t, b0, b1), sub)
+        r = pu.gate(pu.np64(y[b0:b1]), yo, A, dtype)
+        assert r["ok"], ((b0, b1), r)
+
+
+def _all_images_bwd(cfg, dtype, t, g, chunk):
+    for b0 in range(0, cfg.B, chunk):
+        b1 = min(cfg.B, b0 + chunk)
+        sub = gi.with_batch(cfg, b1 - b0)
+        go, A = pu.oracle_bwd(pu._slice(t, b0, b1), sub)
+        for k in ("dx", "dlambda", "du", "dw3", "dh0"):
+            gk = g[k][b0:b1] if k == "dx" else g[k][:, b0:b1]
+            r = pu.gate(pu.np64(gk), go[k], A[k], dtype)
+            assert r["ok"], (k, (b0, b1), r)
+
+
+@pytest.mark.parametrize("name,chunk", [("cfg5_1k", 4), ("cfg3_enc378", 32), ("cfg4_2k", 1)])
+def test_every_image_of_the_full_size_forward(name, chunk):
+    """Full size, launched as bench.py launches it, and EVERY image compared (a tail-wave or CTA-scheduling fault in
+    an image the sampled check skips would pass there)."""
+    cfg = gi.CONFIGS[name]
+    t = gi.make_inputs(cfg, "bf16", device="cuda:0", with_dy=False)
+    y = gspn.gspn_scan_fwd(t["x"], t["w3"], t["lam"], t["u"], cfg.G, cfg.dir_mask)
+    torch.cuda.synchronize()
+    _all_images_fwd(cfg, "bf16", t, y, chunk)
+
+
+@pytest.mark.parametrize("name,chunk", [("cfg5_1k", 4), ("cfg3_enc378", 32)])
+def test_every_image_of_the_full_size_backward(name, chunk):
+    cfg = gi.CONFIGS[name]
+    t = gi.make_inputs(cfg, "bf16", device="cuda:0", with_dy=True)
+    g = gspn.gspn_scan_bwd(t["x"], t["w3"], t["lam"], t["u"], t["dy"], cfg.G, cfg.dir_mask)
+    torch.cuda.synchronize()
+    _all_images_bwd(cfg, "bf16", t, g, chunk)
+
+
+# ---------------------------------------------------------------------------------- aligned benchmark shapes, backward (hole e)
+@pytest.mark.parametrize("shape,dtype", [((1, 8, 128, 128, 2), "bf16"), ((2, 16, 56, 56, 2), "bf16"), ((1, 8, 56, 56, 1), "f32")],
+                         ids=["128x128-cg4-bf16", "56x56-cg8-bf16", "56x56-cg8-f32"])
+def test_auto_backward_on_the_aligned_benchmark_shapes(shape, dtype, record_property):
+    """GSPN_IMPL_AUTO backward at the 2K shape (C/G = 4) and the classification shape (C/G = 8): parity, and the
+    variant that ran is reported; a fall-through to the naive kernel is an expected failure, not a silent pass."""
+    cfg = gi.small_config("ab", *shape, seed=61, backward=True)
+    r = pu.check_bwd(cfg, dtype)
+    assert r["ok"], r
+    record_property("variant", r["variant"])
+    if r["variant"] == "naive_bwd":
+        pytest.xfail("GSPN_IMPL_AUTO has no fused backward for this shape yet (line_bwd is opt-in until it has run on hardware)")
+
+
+# ---------------------------------------------------------------------------------- out-of-grid taps (hole f, reading 3)
+def _poison(t, cfg):
+    """NaN in every tap whose neighbour lies outside the grid (the generator stores 0 there)."""
+    w = t["w3"].clone()
+    for q, d in enumerate(gi.dir_list(cfg.dir_mask)):
+        if d < 2:
+            w[q, :, :, 0, :, 0] = float("nan")
+            w[q, :, :, 2, :, cfg.W - 1] = float("nan")
+        else:
+            w[q, :, :, 0, 0, :] = float("nan")
+            w[q, :, :, 2, cfg.H - 1, :] = float("nan")
+    return w
+
+
+FWD_IMPLS = [("auto", gspn.IMPL_AUTO), ("naive", gspn.IMPL_NAIVE), ("tile", gspn.IMPL_FUSED), ("flat", gspn.IMPL_FLAT),
+             ("chain", gspn.IMPL_CHAIN), ("plane", gspn.IMPL_PLANE), ("line", gspn.IMPL_LINE)]
+
+
+@pytest.mark.parametrize("name,impl", FWD_IMPLS, ids=[n for n, _ in FWD_IMPLS])
+def test_out_of_grid_taps_are_never_read_forward(name, impl):
+    """include/gspn.h: the tap of a neighbour outside the grid is never used, so a NaN stored there cannot leak."""
+    ran = 0
+    for shape in [(1, 4, 16, 16, 2), (2, 4, 27, 27, 1), (1, 2, 40, 24, 1)]:
+        for dtype in ("f32", "bf16"):
+            cfg = gi.small_config("nan", *shape, seed=71)
+            d = {k: v.cuda() for k, v in gi.make_inputs(cfg, dtype).items()}
+            y0 = _try(lambda: gspn.gspn_scan_fwd(d["x"], d["w3"], d["lam"], d["u"], cfg.G, cfg.dir_mask, impl=impl))
+            if y0 is None:
+                continue
+            y1 = gspn.gspn_scan_fwd(d["x"], _poison(d, cfg), d["lam"], d["u"], cfg.G, cfg.dir_mask, impl=impl)
+            assert torch.equal(y0, y1), (shape, dtype)
+            ran += 1
+    assert ran >= 1
+
+
+BWD_IMPLS = [("auto", gspn.IMPL_AUTO), ("naive", gspn.IMPL_NAIVE), ("group", gspn.IMPL_FUSED), ("chain", gspn.IMPL_CHAIN),
+             ("plane", gspn.IMPL_PLANE)]
+
+
+@pytest.mark.parametrize("name,impl", BWD_IMPLS, ids=[n for n, _ in BWD_IMPLS])
+def test_out_of_grid_taps_are_never_read_backward(name, impl):
+    """Every gradient but the dw3 entries of the poisoned taps themselves is unchanged (those entries multiply h
+    outside the grid, which is 0: the kernels write 0 there whatever the tap holds)."""
+    ran = 0
+    for shape in [(1, 4, 16, 16, 2), (2, 4, 27, 27, 1), (1, 2, 40, 24, 1)]:
+        for dtype in ("f32", "bf16"):
+            cfg = gi.small_config("nanb", *shape, seed=72, backward=True)
+            d = {k: v.cuda() for k, v in gi.make_inputs(cfg, dtype, with_dy=True).items()}
+            g0 = _try(lambda: gspn.gspn_scan_bwd(d["x"], d["w3"], d["lam"], d["u"], d["dy"], cfg.G, cfg.dir_mask, impl=impl))
+            if g0 is None:
+                continue
+            g1 = gspn.gspn_scan_bwd(d["x"], _poison(d, cfg), d["lam"], d["u"], d["dy"], cfg.G, cfg.dir_mask, impl=impl)
+            for k in g0:
+                assert torch.equal(g0[k], g1[k]), (shape, dtype, k)
+            ran += 1
+    assert ran >= 1
+
+
+# ---------------------------------------------------------------------------------- run-to-run bit identity (hole g)
+@pytest.mark.parametrize("name,impl", FWD_IMPLS, ids=[n for n, _ in FWD_IMPLS])
+def test_forward_is_bit_identical_run_to_run(name, impl):
+    """compute-sanitizer is closed on this pool; the named-barrier half swaps and the mbarrier hand-offs are checked
+    by repetition instead: five runs on the same operands give the same bits."""
+    ran = 0
+    for shape, dtype in [((4, 8, 73, 73, 2), "bf16"), ((2, 8, 56, 56, 2), "bf16"), ((2, 8, 128, 128, 2), "bf16"),
+                         ((8, 8, 27, 27, 2), "bf16"), ((2, 4, 56, 56, 1), "f32")]:
+        cfg = gi.small_config("rep", *shape, seed=81)
+        d = {k: v.cuda() for k, v in gi.make_inputs(cfg, dtype).items()}
+        y0 = _try(lambda: gspn.gspn_scan_fwd(d["x"], d["w3"], d["lam"], d["u"], cfg.G, cfg.dir_mask, impl=impl))
+        if y0 is None:
+            continue
+        for _ in range(4):
+            y = gspn.gspn_scan_fwd(d["x"], d["w3"], d["lam"], d["u"], cfg.G, cfg.dir_mask, impl=impl)
+            assert torch.equal(y, y0), (shape, dtype)
+        ran += 1
+    assert ran >= 1
+
+
+@pytest.mark.parametrize("name,impl", BWD_IMPLS, ids=[n for n, _ in BWD_IMPLS])
+def test_backward_is_bit_identical_run_to_run(name, impl):
+    ran = 0
+    for shape, dtype in [((4, 8, 73, 73, 2), "bf16"), ((8, 8, 27, 27, 2), "bf16"), ((2, 4, 56, 56, 1), "f32")]:
+        cfg = gi.small_config("repb", *shape, seed=82, backward=True)
+        d = {k: v.cuda() for k, v in gi.make_inputs(cfg, dtype, with_dy=True).items()}
+        g0 = _try(lambda: gspn.gspn_scan_bwd(d["x"], d["w3"], d["lam"], d["u"], d["dy"], cfg.G, cfg.dir_mask, impl=impl))
+        if g0 is None:
+            continue
+        for _ in range(4):
+            g = gspn.gspn_scan_bwd(d["x"], d["w3"], d["lam"], d["u"], d["dy"], cfg.G, cfg.dir_mask, impl=impl)
+            for k in g0:
+                assert torch.equal(g[k], g0[k]), (shape, dtype, k)
+        ran += 1
+    assert ran >= 1
+
+
+# ---------------------------------------------------------------------------------- optional outputs per kernel (ADVICE low)
+@pytest.mark.parametrize("name,impl", BWD_IMPLS, ids=[n for n, _ in BWD_IMPLS])
+@pytest.mark.parametrize("shape", [(1, 4, 8, 8, 2), (1, 4, 40, 44, 2)], ids=["8x8", "40x44"])
+def test_optional_outputs_per_kernel(shape, name, impl):
+    """NULL output pointers (any subset) leave the other outputs bit-identical, for every backward kernel and for
+    lines longer than one warp."""
+    cfg = gi.small_config("opt2", *shape, seed=91, backward=True)
+    t = {k: v.cuda() for k, v in gi.make_inputs(cfg, "f32", with_dy=True).items()}
+    full = _try(lambda: gspn.gspn_scan_bwd(t["x"], t["w3"], t["lam"], t["u"], t["dy"], cfg.G, cfg.dir_mask, impl=impl))
+    if full is None:
+        pytest.skip("shape not held by this kernel")
+    for need in (("dx",), ("dw3",), ("du", "dh0"), ("dlambda", "dw3"), ("dh0",)):
+        part = gspn.gspn_scan_bwd(t["x"], t["w3"], t["lam"], t["u"], t["dy"], cfg.G, cfg.dir_mask, need=need, impl=impl)
+        assert set(part) == set(need)
+        for k in need:
+            assert torch.equal(part[k], full[k]), (need, k)
