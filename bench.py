@@ -203,6 +203,23 @@ def run_reference(args):
     }))
 
 
+def traffic_of(key: str):
+    """DRAM bytes per launch of a kernel from its committed `ncu --set full` capture (profiles/traffic.json), or None
+    when there is no capture or the kernel's source file has changed since (sha1 recorded beside the bytes)."""
+    import hashlib
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            e = json.load(f).get(key)
+        if not isinstance(e, dict):
+            return None
+        with open(os.path.join(ROOT, "paper_2606_00746_b200", "csrc", e["source"]), "rb") as f:
+            if hashlib.sha1(f.read()).hexdigest() != e["sha1"]:
+                return None
+        return float(e["bytes"])
+    except Exception:
+        return None
+
+
 def time_cpu_oracle(cfg, dtype, budget_s=12.0):
     """cpu_baseline leg: the oracle (fp32 build) on the workload, repeated within a time budget."""
     import gspn_inputs as gi
@@ -220,17 +237,46 @@ def time_cpu_oracle(cfg, dtype, budget_s=12.0):
             orc.bwd(a["x"], a["w3"], a["lam"], a["u"], a["dy"], cfg.G, cfg.dir_mask)
         times.append(time.perf_counter() - t0)
     dt = min(times[1:]) if len(times) > 1 else times[0]
-    return {"value": nbytes / dt / 1e9, "unit": "GB/s", "cores": orc.threads(), "kind": "oracle",
+    # the plain single-thread oracle beside the OpenMP one, on a bounded sample (one image)
+    single = None
+    try:
+        nthr = orc.threads()
+        sub1 = gi.with_batch(cfg, 1)
+        a1 = {k: (v[:1] if k in ("x", "dy") else v[:, :1]) for k, v in a.items()}
+        a1 = {k: __import__("numpy").ascontiguousarray(v) for k, v in a1.items()}
+        orc.set_threads(1)
+        t0 = time.perf_counter()
+        orc.fwd(a1["x"], a1["w3"], a1["lam"], a1["u"], cfg.G, cfg.dir_mask)
+        if cfg.backward:
+            orc.bwd(a1["x"], a1["w3"], a1["lam"], a1["u"], a1["dy"], cfg.G, cfg.dir_mask)
+        d1 = time.perf_counter() - t0
+        orc.set_threads(nthr)
+        n1 = sub1.fwd_bytes(s) + (sub1.bwd_bytes(s) if cfg.backward else 0)
+        single = {"value": n1 / d1 / 1e9, "unit": "GB/s", "cores": 1, "ms_per_image": d1 * 1e3,
+                  "sample": f"image 0 of {cfg.name}, one thread"}
+    except Exception as e:      # pragma: no cover
+        single = {"error": repr(e)}
+    return {"value": nbytes / dt / 1e9, "unit": "GB/s", "cores": orc.threads(), "kind": "oracle", "single_thread": single,
             "ms_per_step": dt * 1e3, "pxch_per_s": cfg.n / dt,
             "sample": f"full workload {cfg.name} (B={cfg.B}), fp32 build, fwd{'+bwd' if cfg.backward else ''}, "
                       f"best of {len(times) - 1} after 1 warm-up"}
 
 
 # ------------------------------------------------------------------------------------------------
+def l2_bytes(torch) -> int:
+    return int(getattr(torch.cuda.get_device_properties(torch.cuda.current_device()), "L2_cache_size", 126 << 20))
+
+
 def time_config(gspn, torch, cfg, dtype, steps, warmup, world, impl, want_bwd, tensors=None):
     """Times `steps` steps (fwd [+ bwd]) of cfg with CUDA events on the launching stream.
+    Operands that do not exceed twice the L2 size are flushed out of it before every timed step (a buffer larger than
+    L2 is overwritten, outside the event windows); the step time is then the sum of the per-kernel windows.
     Returns (dict of timings, tensors, last outputs)."""
     dev = torch.device("cuda", torch.cuda.current_device())
+    s_ = 4 if dtype == "f32" else 2
+    op_bytes = cfg.fwd_bytes(s_) + (cfg.bwd_bytes(s_) if want_bwd else 0)
+    flush = op_bytes <= 2 * l2_bytes(torch)
+    fbuf = torch.empty(2 * l2_bytes(torch), dtype=torch.uint8, device=dev) if flush else None
     if tensors is None:
         tensors = __import__("gspn_inputs").make_inputs(cfg, dtype, device=dev, with_dy=want_bwd)
     t = tensors
@@ -241,6 +287,8 @@ def time_config(gspn, torch, cfg, dtype, steps, warmup, world, impl, want_bwd, t
     def step(record=None):
         nonlocal grads, launches
         if record:
+            if flush:
+                fbuf.fill_(1)
             record[0].record()
         gspn.gspn_scan_fwd(t["x"], t["w3"], t["lam"], t["u"], cfg.G, cfg.dir_mask, out=y, impl=impl)
         launches += gspn.gspn_last_launch_count()
@@ -269,8 +317,11 @@ def time_config(gspn, torch, cfg, dtype, steps, warmup, world, impl, want_bwd, t
     total_ms = ev[0][0].elapsed_time(ev[-1][2])
     fwd_ms = sorted(e[0].elapsed_time(e[1]) for e in ev)
     bwd_ms = sorted(e[1].elapsed_time(e[2]) for e in ev) if want_bwd else None
+    if flush:       # the flushes sit between the event windows: the step is the sum of its kernels' windows
+        total_ms = sum(fwd_ms) + (sum(bwd_ms) if want_bwd else 0.0)
     total_ms = max_over_ranks(total_ms, world, dev)
-    res = {"total_ms": total_ms, "ms_per_step": total_ms / steps, "wall_ms": wall * 1e3,
+    res = {"total_ms": total_ms, "ms_per_step": total_ms / steps, "wall_ms": wall * 1e3, "l2_flush": flush,
+           "operand_bytes": op_bytes,
            "fwd_ms_mean": sum(fwd_ms) / steps, "fwd_ms_median": fwd_ms[steps // 2], "fwd_ms_min": fwd_ms[0],
            "launches": launches, "variant_fwd": vf, "variant_bwd": vb}
     if want_bwd:
@@ -365,13 +416,7 @@ def main():
                           "gbs": bwd_b / (res["bwd_ms_mean"] * 1e-3) / 1e9,
                           "frac": bwd_b / (res["bwd_ms_mean"] * 1e-3) / 1e9 / peak}
     dom = max(kernels, key=lambda k: kernels[k]["ms_mean"])
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")      # written by hand from an `ncu --set full` capture
-    try:
-        with open(tpath) as f:
-            traffic = json.load(f).get(f"{cfg.name}:{dtype}:{kernels[dom]['variant']}")
-    except Exception:
-        pass
+    traffic = traffic_of(f"{cfg.name}:{dtype}:{kernels[dom]['variant']}")
     roofline = {"bound": "hbm", "kernel": kernels[dom]["variant"], "pass": dom,
                 "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s", "frac": kernels[dom]["frac"],
                 "traffic": traffic, "peak_source": peak_src,
@@ -389,10 +434,17 @@ def main():
 
     e2e = None
     if not args.no_e2e:
-        ms, h2d, d2h, _, _, n_e2e = time_e2e(gspn, torch, cfg, dtype, steps, warmup, world, want_bwd, tensors)
+        ms, h2d, d2h, ye, oute, n_e2e = time_e2e(gspn, torch, cfg, dtype, steps, warmup, world, want_bwd, tensors)
         e2e = {"value": world * step_bytes / (ms * 1e-3) / 1e9, "unit": "GB/s", "ms_per_step": ms,
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e,
                "api": "gspn_scan_fwd_host" + (" + gspn_scan_bwd_host" if want_bwd else "")}
+        if not args.no_parity and rank == 0:      # the host path's own outputs are gated too, not only the device path's
+            import parity_util as pu
+            pe = pu.check_fwd_sampled(cfg, dtype, tensors, ye)
+            e2e["parity"] = {"fwd_ok": pe["ok"]}
+            if want_bwd:
+                e2e["parity"]["bwd_ok"] = pu.check_bwd_sampled(cfg, dtype, tensors, oute)["ok"]
+        del ye, oute
     del grads, y
 
     others = None
@@ -405,21 +457,21 @@ def main():
                 if name == cfg.name and dt == dtype:
                     continue
                 so = 4 if dt == "f32" else 2
-                # the backward of the other configs is timed where a fused single-launch kernel holds the unit on chip
-                # (C/G <= 4 and the fp32 dx planes of a unit within shared memory): the tiny and the 378-px configs
-                ob = impl == gspn.IMPL_AUTO and oc.C // oc.G <= 4 and (oc.C // oc.G) * oc.H * oc.W * 4 <= 100 * 1024
+                # the backward of every other config is timed too, with whatever kernel GSPN_IMPL_AUTO picks (the variant
+                # is printed: a naive fall-through shows)
+                ob = impl == gspn.IMPL_AUTO
                 r, tt, yy, gg = time_config(gspn, torch, oc, dt, max(5, min(steps, 20)), 3, 1, impl, ob)
                 if ob:
                     bb = oc.bwd_bytes(so)
                     others[f"{name}:{dt}:bwd"] = {"variant": r["variant_bwd"], "ms": r["bwd_ms_mean"], "ms_min": r["bwd_ms_min"],
                                                    "gbs": bb / (r["bwd_ms_mean"] * 1e-3) / 1e9,
                                                    "frac": bb / (r["bwd_ms_mean"] * 1e-3) / 1e9 / peak,
-                                                   "pxch_per_s": oc.n / (r["bwd_ms_mean"] * 1e-3)}
+                                                   "pxch_per_s": oc.n / (r["bwd_ms_mean"] * 1e-3), "l2_flush": r["l2_flush"]}
                 fb = oc.fwd_bytes(so)
                 others[f"{name}:{dt}:fwd"] = {"variant": r["variant_fwd"], "ms": r["fwd_ms_mean"], "ms_min": r["fwd_ms_min"],
                                                "gbs": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9,
                                                "frac": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9 / peak,
-                                               "pxch_per_s": oc.n / (r["fwd_ms_mean"] * 1e-3)}
+                                               "pxch_per_s": oc.n / (r["fwd_ms_mean"] * 1e-3), "l2_flush": r["l2_flush"]}
                 del tt, yy, gg
                 torch.cuda.empty_cache()
         # the fused Eq. 3 normalisation of the tap logits and its adjoint on every config
@@ -458,7 +510,9 @@ def main():
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": cfg.name, "B": cfg.B, "C": cfg.C, "H": cfg.H, "W": cfg.W, "G": cfg.G,
                        "dir_mask": cfg.dir_mask, "storage": dtype, "pass": "fwd+bwd" if want_bwd else "fwd",
-                       "l2": f"operands {step_bytes / 1e6:.0f} MB per step > 126 MB L2 (no flush needed)",
+                       "l2": (f"operands {step_bytes / 1e6:.0f} MB per step <= 2 x {l2_bytes(torch) >> 20} MB L2: a "
+                              f"{2 * l2_bytes(torch) >> 20} MB buffer is overwritten before every timed step" if res["l2_flush"]
+                              else f"operands {step_bytes / 1e6:.0f} MB per step > 2 x {l2_bytes(torch) >> 20} MB L2 (no flush needed)"),
                        "per_rank_batch": cfg.B},
             "frac_of_peak": value / world / peak, "pxch_per_s": world * cfg.n / (res["ms_per_step"] * 1e-3),
             "kernels": kernels, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,

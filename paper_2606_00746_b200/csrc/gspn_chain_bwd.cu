@@ -736,7 +736,7 @@ static size_t chain_bwd_layout(const Shape& sh, int es, int P, int NSV, int NSH,
 template <typename ST, int P>
 static int launch_chain_bwd(const ChainBwdParams& prm, int items, int threads, cudaStream_t st) {
     auto kern = chain_bwd_kernel<ST, P>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prm.total);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("chain bwd: cudaFuncSetAttribute(%u B): %s", prm.total, cudaGetErrorString(e)); return GSPN_ECUDA; }
     kern<<<items, threads, prm.total, st>>>(prm);
     e = cudaGetLastError();

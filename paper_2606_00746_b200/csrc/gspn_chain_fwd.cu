@@ -377,7 +377,7 @@ static size_t chain_fwd_layout(const Shape& sh, int es, int P, int NC, int NSV, 
 template <typename ST, int P, int CBH>
 static int launch_chain_fwd(const ChainFwdParams& prm, int items, int threads, cudaStream_t st) {
     auto kern = chain_fwd_kernel<ST, P, CBH>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prm.total);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("chain fwd: cudaFuncSetAttribute(%u B): %s", prm.total, cudaGetErrorString(e)); return GSPN_ECUDA; }
     kern<<<items, threads, prm.total, st>>>(prm);
     e = cudaGetLastError();

@@ -456,7 +456,7 @@ static size_t flat_layout(const Shape& sh, int es, int P, int nch, int Kv, int N
 template <typename ST, int P, int CS>
 static int launch_flat(const FlatPlan& pl, int items, cudaStream_t st) {
     auto kern = fwd_flat_kernel<ST, P, CS>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("flat fwd: cudaFuncSetAttribute(%zu B): %s", pl.smem, cudaGetErrorString(e)); return GSPN_ECUDA; }
     kern<<<items, pl.threads, pl.smem, st>>>(pl.prm);
     e = cudaGetLastError();

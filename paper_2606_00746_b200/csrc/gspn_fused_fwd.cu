@@ -403,7 +403,7 @@ static int launch_tile(const FwdArgs<ST>& a, const TilePlan& pl, cudaStream_t st
         if (!encode_tensor_map(&m[4 + t], ES, const_cast<void*>(src[t].p), 4, dh, shh, bh)) return GSPN_ECUDA;
     }
     auto kern = fwd_tile_kernel<ST, CPTB, R>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("fused fwd: cudaFuncSetAttribute(%zu B): %s", pl.smem, cudaGetErrorString(e)); return GSPN_ECUDA; }
     const int items = sh.B * sh.G * (sh.cg() / cpc);
     const int threads = (4 + 4 * cpc) * 32;

@@ -512,18 +512,30 @@ static int line_fwd_run(const FwdArgs<ST>& a, cudaStream_t st) {
     struct Src { const void* p; uint64_t planes; };
     const Src src[4] = {{a.x, (uint64_t)sh.B * sh.C}, {a.w3, (uint64_t)D * sh.B * sh.G * 3},
                         {a.lam, (uint64_t)D * sh.B * sh.C}, {a.u, (uint64_t)D * sh.B * sh.C}};
-    CUtensorMap m[8];
-    const uint64_t row_b = (uint64_t)W * ES, plane_b = (uint64_t)H * W * ES;
-    for (int t = 0; t < 4; ++t) {
-        const uint64_t dv[3] = {(uint64_t)W, (uint64_t)H, src[t].planes};
-        const uint64_t sv[2] = {row_b, plane_b};
-        const uint32_t np = prm.multi ? (t == 1 ? 3u : (uint32_t)NC) : 1u;      // planes per box
-        const uint32_t bv[3] = {(uint32_t)W, (uint32_t)S, np};
-        if (!encode_tensor_map(&m[t], ES, const_cast<void*>(src[t].p), 3, dv, sv, bv)) return GSPN_ECUDA;
-        // column stages: a box is 32 bytes wide and the whole plane height; SWIZZLE_32B keeps the lanes' 16-byte reads
-        // (one row per lane) free of bank conflicts
-        const uint32_t bh[3] = {(uint32_t)(2 * K), (uint32_t)H, np};
-        if (!encode_tensor_map(&m[4 + t], ES, const_cast<void*>(src[t].p), 3, dv, sv, bh, 1)) return GSPN_ECUDA;
+    // The eight tensor maps depend on the operand addresses and the shape only: the last set of this host thread is kept
+    // (a cached launch descriptor, include/gspn.h) so that repeated calls on the same buffers skip the driver's encoder.
+    struct MapCache { const void* p[4]; int B, C, H, W, G, multi; CUtensorMap m[8]; bool valid; };
+    static thread_local MapCache mc{};
+    const bool hit = mc.valid && mc.p[0] == a.x && mc.p[1] == a.w3 && mc.p[2] == a.lam && mc.p[3] == a.u && mc.B == sh.B &&
+                     mc.C == sh.C && mc.H == H && mc.W == W && mc.G == (int)(sh.G * 16 + NC) && mc.multi == prm.multi * 8 + D;
+    CUtensorMap* const m = mc.m;
+    if (!hit) {
+        mc.valid = false;
+        const uint64_t row_b = (uint64_t)W * ES, plane_b = (uint64_t)H * W * ES;
+        for (int t = 0; t < 4; ++t) {
+            const uint64_t dv[3] = {(uint64_t)W, (uint64_t)H, src[t].planes};
+            const uint64_t sv[2] = {row_b, plane_b};
+            const uint32_t np = prm.multi ? (t == 1 ? 3u : (uint32_t)NC) : 1u;      // planes per box
+            const uint32_t bv[3] = {(uint32_t)W, (uint32_t)S, np};
+            if (!encode_tensor_map(&m[t], ES, const_cast<void*>(src[t].p), 3, dv, sv, bv)) return GSPN_ECUDA;
+            // column stages: a box is 32 bytes wide and the whole plane height; SWIZZLE_32B keeps the lanes' 16-byte
+            // reads (one row per lane) free of bank conflicts
+            const uint32_t bh[3] = {(uint32_t)(2 * K), (uint32_t)H, np};
+            if (!encode_tensor_map(&m[4 + t], ES, const_cast<void*>(src[t].p), 3, dv, sv, bh, 1)) return GSPN_ECUDA;
+        }
+        mc.p[0] = a.x; mc.p[1] = a.w3; mc.p[2] = a.lam; mc.p[3] = a.u;
+        mc.B = sh.B; mc.C = sh.C; mc.H = H; mc.W = W; mc.G = (int)(sh.G * 16 + NC); mc.multi = prm.multi * 8 + D;
+        mc.valid = true;
     }
     auto kern = line_fwd_kernel<ST, NC, P>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);

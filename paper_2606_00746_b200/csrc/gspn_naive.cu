@@ -242,7 +242,7 @@ static int prep_smem(K kernel, size_t bytes, const char* what) {
         set_error("%s: needs %zu B of shared memory per CTA (> %d)", what, bytes, kMaxSmemOptin);
         return GSPN_EUNSUPPORTED;
     }
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) {
         set_error("%s: cudaFuncSetAttribute: %s", what, cudaGetErrorString(e));
         return GSPN_ECUDA;

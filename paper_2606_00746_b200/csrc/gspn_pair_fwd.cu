@@ -629,7 +629,7 @@ static size_t plane_fwd_layout(const Shape& sh, int es, int P, int NC, PairFwdPa
 template <typename ST, int P, int NC, int NCW>
 static int launch_plane_fwd(const PairFwdParams& prm, int items, cudaStream_t st) {
     auto kern = plane_fwd_kernel<ST, P, NC, NCW>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prm.total);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("plane fwd: cudaFuncSetAttribute(%u B): %s", prm.total, cudaGetErrorString(e)); return GSPN_ECUDA; }
     kern<<<items, 32 * (4 * (NC / NCW) + 1), prm.total, st>>>(prm);
     e = cudaGetLastError();
@@ -723,7 +723,7 @@ static size_t pair_fwd_layout(const Shape& sh, int es, int P, int NC, PairFwdPar
 template <typename ST, int P, int NC>
 static int launch_pair_fwd(const PairFwdParams& prm, int items, cudaStream_t st) {
     auto kern = pair_fwd_kernel<ST, P, NC>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prm.total);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("pair fwd: cudaFuncSetAttribute(%u B): %s", prm.total, cudaGetErrorString(e)); return GSPN_ECUDA; }
     kern<<<items, 128, prm.total, st>>>(prm);
     e = cudaGetLastError();

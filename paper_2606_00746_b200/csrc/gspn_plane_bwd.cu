@@ -338,7 +338,7 @@ static size_t plane_bwd_layout(const Shape& sh, int es, int NC, PlaneBwdParams* 
 template <typename ST, int NC>
 static int launch_plane_bwd(const PlaneBwdParams& prm, int items, cudaStream_t st) {
     auto kern = plane_bwd_kernel<ST, NC>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prm.total);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("plane bwd: cudaFuncSetAttribute(%u B): %s", prm.total, cudaGetErrorString(e)); return GSPN_ECUDA; }
     kern<<<items, NC >= 2 ? 288 : 160, prm.total, st>>>(prm);
     e = cudaGetLastError();
