@@ -510,9 +510,9 @@ __device__ __forceinline__ void bwd_dir_h(BwdCtx& cx, const bool rev, const bool
                 float dxv[P][4], dlv[P][4], duv[P][4];
                 if (acc) {
 #pragma unroll
-                    for (int k = 0; k < P; ++k) tm_ld<4>(cx.tb + k * 32 * P + j0, dxv[k]);
+                    for (int k = 0; k < P; ++k) if (32 * k < H) tm_ld<4>(cx.tb + k * 32 * P + j0, dxv[k]);   // slots past the plane own no columns
 #pragma unroll
-                    for (int k = 0; k < P; ++k) tm_wait_ld<4>(dxv[k]);
+                    for (int k = 0; k < P; ++k) if (32 * k < H) tm_wait_ld<4>(dxv[k]);
                 }
 #pragma unroll
                 for (int t = 3; t >= 0; --t) {
@@ -549,7 +549,7 @@ __device__ __forceinline__ void bwd_dir_h(BwdCtx& cx, const bool rev, const bool
                 }
 #pragma unroll
                 for (int k = 0; k < P; ++k) {
-                    tm_st<4>(cx.tb + k * 32 * P + j0, dxv[k]);
+                    if (32 * k < H) tm_st<4>(cx.tb + k * 32 * P + j0, dxv[k]);
                     if (lane + 32 * k < H) {
                         const uint32_t off = sub_off<ST>(lane + 32 * k, q, H);
                         bwd_store<ST, 4>(reinterpret_cast<ST*>(ob + (size_t)(PL::ODLAM + c) * pb + off), dlv[k]);
@@ -732,6 +732,7 @@ line_bwd_kernel(const __grid_constant__ BwdMaps mv, const __grid_constant__ BwdM
 #pragma unroll
                 for (int k = 0; k < P; ++k) {
                     const int i = lane + 32 * k;
+                    if (32 * k >= H) continue;
                     for (int jc = 0; jc * K < W; ++jc) {
                         float f[K];
                         tm_ld<K>(cx.tb + k * 32 * P + jc * K, f);

@@ -199,7 +199,7 @@ __device__ __forceinline__ void line_fwd_hstage(const LineCtx& cx, const unsigne
             float yv[P][4];
             if (acc) {
 #pragma unroll
-                for (int k = 0; k < P; ++k) tm_ld<4>(cx.tb + k * 32 * P + j0, yv[k]);
+                for (int k = 0; k < P; ++k) if (32 * k < H) tm_ld<4>(cx.tb + k * 32 * P + j0, yv[k]);   // slots past the plane own no columns
             }
 #pragma unroll
             for (int tt = 0; tt < 4; ++tt) {
@@ -223,7 +223,7 @@ __device__ __forceinline__ void line_fwd_hstage(const LineCtx& cx, const unsigne
                 }
                 if (tt == 0 && acc) {
 #pragma unroll
-                    for (int k = 0; k < P; ++k) tm_wait_ld<4>(yv[k]);
+                    for (int k = 0; k < P; ++k) if (32 * k < H) tm_wait_ld<4>(yv[k]);
                 }
 #pragma unroll
                 for (int k = 0; k < P; ++k) {
@@ -232,7 +232,7 @@ __device__ __forceinline__ void line_fwd_hstage(const LineCtx& cx, const unsigne
                 }
             }
 #pragma unroll
-            for (int k = 0; k < P; ++k) tm_st<4>(cx.tb + k * 32 * P + j0, yv[k]);
+            for (int k = 0; k < P; ++k) if (32 * k < H) tm_st<4>(cx.tb + k * 32 * P + j0, yv[k]);
         }
     }
 }
@@ -447,6 +447,7 @@ line_fwd_kernel(const __grid_constant__ CUtensorMap mxv, const __grid_constant__
 #pragma unroll
             for (int k = 0; k < P; ++k) {
                 const int i = lane + 32 * k;
+                if (32 * k >= H) continue;
                 for (int jc = d; jc * K < W; jc += 2) {
                     float f[K];
                     tm_ld<K>(cx.tb + k * 32 * P + jc * K, f);
