@@ -510,7 +510,10 @@ __device__ __forceinline__ void bwd_dir_h(BwdCtx& cx, const bool rev, const bool
                 float dxv[P][4], dlv[P][4], duv[P][4];
                 if (acc) {
 #pragma unroll
-                    for (int k = 0; k < P; ++k) if (32 * k < H) tm_ld<4>(cx.tb + k * 32 * P + j0, dxv[k]);   // slots past the plane own no columns
+                    for (int k = 0; k < P; ++k) {
+                        if (32 * k < H) tm_ld<4>(cx.tb + k * 32 * P + j0, dxv[k]);  // slots past the plane own no columns
+                        else dxv[k][0] = dxv[k][1] = dxv[k][2] = dxv[k][3] = 0.f;
+                    }
 #pragma unroll
                     for (int k = 0; k < P; ++k) if (32 * k < H) tm_wait_ld<4>(dxv[k]);
                 }

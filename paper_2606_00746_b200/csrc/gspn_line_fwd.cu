@@ -199,7 +199,10 @@ __device__ __forceinline__ void line_fwd_hstage(const LineCtx& cx, const unsigne
             float yv[P][4];
             if (acc) {
 #pragma unroll
-                for (int k = 0; k < P; ++k) if (32 * k < H) tm_ld<4>(cx.tb + k * 32 * P + j0, yv[k]);   // slots past the plane own no columns
+                for (int k = 0; k < P; ++k) {
+                    if (32 * k < H) tm_ld<4>(cx.tb + k * 32 * P + j0, yv[k]);      // slots past the plane own no columns
+                    else yv[k][0] = yv[k][1] = yv[k][2] = yv[k][3] = 0.f;
+                }
             }
 #pragma unroll
             for (int tt = 0; tt < 4; ++tt) {
