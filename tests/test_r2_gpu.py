@@ -230,3 +230,35 @@ def test_optional_outputs_per_kernel(shape, name, impl):
         assert set(part) == set(need)
         for k in need:
             assert torch.equal(part[k], full[k]), (need, k)
+
+
+# ---------------------------------------------------------------------------------- the group backward
+GROUP_SHAPES = [(1, 4, 27, 27, 1), (2, 4, 8, 8, 2), (1, 2, 40, 44, 2), (1, 4, 33, 35, 1), (1, 2, 100, 36, 1)]
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("shape", GROUP_SHAPES, ids=["x".join(map(str, s)) for s in GROUP_SHAPES])
+def test_group_backward_forced(shape, dtype):
+    """fused_bwd_group sits in GSPN_IMPL_AUTO's fall-back chain but no round-1 test forced it: parity with masks and h0."""
+    ran = 0
+    for mask in (15, 6, 9):
+        cfg = gi.small_config("grp", *shape, dir_mask=mask, seed=95 + mask, backward=True)
+        r = _try(lambda: pu.check_bwd(cfg, dtype, impl=gspn.IMPL_FUSED, with_h0=True))
+        if r is None:
+            continue
+        assert r["ok"] and r["variant"] == "fused_bwd_group", (mask, r)
+        ran += 1
+    if not ran:
+        pytest.skip("shape not held by the group kernel")
+
+
+@pytest.mark.parametrize("shape,dtype", [((1, 4, 27, 27, 1), "f32"), ((1, 2, 144, 144, 2), "bf16")], ids=["27x27-cg4-f32", "144x144-cg1-bf16"])
+def test_auto_backward_fallback_shapes(shape, dtype, record_property):
+    """Shapes the preferred backward kernels refuse (plane: fp32 planes beyond shared memory; chain: lines beyond 128):
+    AUTO must still return oracle-exact gradients, whatever it lands on; the variant is recorded."""
+    cfg = gi.small_config("fb", *shape, seed=97, backward=True)
+    r = _try(lambda: pu.check_bwd(cfg, dtype, with_h0=True))
+    if r is None:
+        pytest.xfail("no backward kernel under GSPN_IMPL_AUTO holds this shape")
+    record_property("variant", r["variant"])
+    assert r["ok"], r
