@@ -648,27 +648,26 @@ line_bwd_kernel(const __grid_constant__ BwdMaps mv, const __grid_constant__ BwdM
             const int q = prm.slab[dir];
             const BwdMaps& mm = vert ? mv : mh;
             const int pw = ((q * prm.B + b) * prm.G + g) * 3, pc = (q * prm.B + b) * prm.C + c0, px = b * prm.C + c0;
-            // this lane's box: operand map, first plane in its tensor, plane slot in the stage, pass-1 member?
-            const CUtensorMap* map = nullptr;
-            int plane = 0, slot = 0;
-            bool in1 = false, issue = false;
-            if (prm.multi) {
-                issue = lane < 5;
-                if (lane == 0) { map = &mm.lw; plane = pw; slot = 0; in1 = true; }
-                else if (lane == 1) { map = &mm.ll; plane = pc; slot = PL::LAM; in1 = true; }
-                else if (lane == 2) { map = &mm.lx; plane = px; slot = PL::X; in1 = true; }
-                else if (lane == 3) { map = &mm.lu; plane = pc; slot = PL::U; }
-                else if (lane == 4) { map = &mm.ldy; plane = px; slot = PL::DY; }
-            } else {
-                issue = lane < PL::N2;
-                slot = lane;
-                in1 = lane < PL::N1;
-                if (lane < 3) { map = &mm.lw; plane = pw + lane; }
-                else if (lane < PL::X) { map = &mm.ll; plane = pc + lane - PL::LAM; }
-                else if (lane < PL::U) { map = &mm.lx; plane = px + lane - PL::X; }
-                else if (lane < PL::DY) { map = &mm.lu; plane = pc + lane - PL::U; }
-                else if (lane < PL::N2) { map = &mm.ldy; plane = px + lane - PL::DY; }
-            }
+            // box number n of a stage: operand map, first plane in its tensor, plane slot in the stage, pass-1 member?
+            // (multi: 5 boxes, one per operand; else one per plane: up to 3 + 4 NC = 35, more than a warp has lanes)
+            const int nbox = prm.multi ? 5 : PL::N2;
+            auto box = [&](int n, const CUtensorMap*& map, int& plane, int& slot, bool& in1) {
+                if (prm.multi) {
+                    if (n == 0) { map = &mm.lw; plane = pw; slot = 0; in1 = true; }
+                    else if (n == 1) { map = &mm.ll; plane = pc; slot = PL::LAM; in1 = true; }
+                    else if (n == 2) { map = &mm.lx; plane = px; slot = PL::X; in1 = true; }
+                    else if (n == 3) { map = &mm.lu; plane = pc; slot = PL::U; in1 = false; }
+                    else { map = &mm.ldy; plane = px; slot = PL::DY; in1 = false; }
+                } else {
+                    slot = n;
+                    in1 = n < PL::N1;
+                    if (n < 3) { map = &mm.lw; plane = pw + n; }
+                    else if (n < PL::X) { map = &mm.ll; plane = pc + n - PL::LAM; }
+                    else if (n < PL::U) { map = &mm.lx; plane = px + n - PL::X; }
+                    else if (n < PL::DY) { map = &mm.lu; plane = pc + n - PL::U; }
+                    else { map = &mm.ldy; plane = px + n - PL::DY; }
+                }
+            };
             const int Ls = vert ? H : W, Lc = vert ? W : H;
             const int nblk = (Ls + S - 1) / S;
             const uint32_t plane_tx = (uint32_t)(S * ES) * (uint32_t)Lc;       // bytes one plane brings per stage
@@ -679,11 +678,17 @@ line_bwd_kernel(const __grid_constant__ BwdMaps mv, const __grid_constant__ BwdM
                     if (it >= NS) mbar_wait(&empty[stg], ((it / NS) - 1) & 1);
                     if (lane == 0) mbar_arrive_expect_tx(&full[stg], plane_tx * (pass ? PL::N2 : PL::N1));
                     __syncwarp();
-                    if (issue && (pass || in1)) {
-                        unsigned char* dst = ring + (size_t)stg * stage_bytes + (size_t)slot * prm.pb;
-                        const int s0 = rev ? Ls - (blk + 1) * S : blk * S;
-                        if (vert) tma_load_3d(dst, map, 0, s0, plane, &full[stg]);
-                        else tma_load_4d(dst, map, 0, 0, s0 / K, plane, &full[stg]);
+                    const int s0 = rev ? Ls - (blk + 1) * S : blk * S;
+                    for (int bx = lane; bx < nbox; bx += 32) {
+                        const CUtensorMap* map = nullptr;
+                        int plane = 0, slot = 0;
+                        bool in1 = false;
+                        box(bx, map, plane, slot, in1);
+                        if (pass || in1) {
+                            unsigned char* dst = ring + (size_t)stg * stage_bytes + (size_t)slot * prm.pb;
+                            if (vert) tma_load_3d(dst, map, 0, s0, plane, &full[stg]);
+                            else tma_load_4d(dst, map, 0, 0, s0 / K, plane, &full[stg]);
+                        }
                     }
                 }
         }
