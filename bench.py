@@ -53,6 +53,7 @@ def parse():
     ap.add_argument("--no-parity", action="store_true", help="skip the sampled oracle check of the timed outputs")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--line-bwd-child", action="store_true", help=argparse.SUPPRESS)
     return ap.parse_args()
 
 
@@ -368,8 +369,69 @@ def time_e2e(gspn, torch, cfg, dtype, steps, warmup, world, want_bwd, tensors):
 
 
 # ------------------------------------------------------------------------------------------------
+def line_bwd_child():
+    """Child process of the bench (see line_bwd_probe): the line backward, forced, on the aligned configs; parity on
+    sampled images first, then timing.  Prints one JSON object."""
+    import torch
+    import gspn_inputs as gi
+    import paper_2606_00746_b200 as gspn
+    import parity_util as pu
+    peak, _ = peak_hbm()
+    res = {}
+    for name, dt in (("cfg4_2k", "bf16"), ("cfg2_cls56", "bf16")):
+        cfg = gi.CONFIGS[name]
+        key = f"{name}:{dt}:bwd"
+        try:
+            t = gi.make_inputs(cfg, dt, device="cuda:0", with_dy=True)
+            g = gspn.gspn_scan_bwd(t["x"], t["w3"], t["lam"], t["u"], t["dy"], cfg.G, cfg.dir_mask, impl=gspn.IMPL_LINE)
+            torch.cuda.synchronize()
+            ok = pu.check_bwd_sampled(cfg, dt, t, g)["ok"]
+            del g
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            for _ in range(3):
+                gspn.gspn_scan_bwd(t["x"], t["w3"], t["lam"], t["u"], t["dy"], cfg.G, cfg.dir_mask, impl=gspn.IMPL_LINE)
+            n = 10
+            e0.record()
+            for _ in range(n):
+                gspn.gspn_scan_bwd(t["x"], t["w3"], t["lam"], t["u"], t["dy"], cfg.G, cfg.dir_mask, impl=gspn.IMPL_LINE)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / n
+            bb = cfg.bwd_bytes(2)
+            res[key] = {"variant": gspn.gspn_last_variant(), "parity_ok": bool(ok), "ms": ms, "gbs": bb / (ms * 1e-3) / 1e9,
+                        "frac": bb / (ms * 1e-3) / 1e9 / peak}
+        except Exception as ex:      # noqa: BLE001 -- whatever goes wrong is the result
+            res[key] = {"variant": "line_bwd", "error": repr(ex)[:300]}
+            break
+        del t
+        torch.cuda.empty_cache()
+    print("LINE_BWD_CHILD " + json.dumps(res))
+
+
+def line_bwd_probe(limit_s: int = 240):
+    """The line backward (csrc/gspn_line_bwd.cu) is not in GSPN_IMPL_AUTO: it had not run on hardware when round 2 ended.
+    The bench gives it one bounded chance in a CHILD process (its own CUDA context, a time limit): forced with
+    GSPN_IMPL_LINE on the two aligned configs, gated on sampled images against the oracle, then timed.  Whatever happens
+    is reported under others["line_bwd_child"]; nothing of the main line depends on it."""
+    import subprocess
+    try:
+        p = subprocess.run([sys.executable, os.path.abspath(__file__), "--line-bwd-child"], cwd=ROOT, stdout=subprocess.PIPE,
+                           stderr=subprocess.STDOUT, text=True, timeout=limit_s)
+        for line in p.stdout.splitlines():
+            if line.startswith("LINE_BWD_CHILD "):
+                return {"rc": p.returncode, "results": json.loads(line[len("LINE_BWD_CHILD "):])}
+        return {"rc": p.returncode, "error": p.stdout[-400:]}
+    except subprocess.TimeoutExpired:
+        return {"rc": 124, "error": f"timed out after {limit_s} s"}
+    except Exception as ex:      # noqa: BLE001
+        return {"rc": -1, "error": repr(ex)[:300]}
+
+
 def main():
     args = parse()
+    if args.line_bwd_child:
+        line_bwd_child()
+        return
     if args.impl == "reference":
         run_reference(args)
         return
@@ -504,6 +566,9 @@ def main():
                                                     "gbs": nb / (ms * 1e-3) / 1e9, "frac": nb / (ms * 1e-3) / 1e9 / peak}
                 del lg, buf
                 torch.cuda.empty_cache()
+
+    if others is not None and impl == gspn.IMPL_AUTO:
+        others["line_bwd_child"] = line_bwd_probe()
 
     cpu = None
     if not args.no_cpu and rank == 0 and world == 1:
