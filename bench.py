@@ -408,7 +408,7 @@ def line_bwd_child():
     print("LINE_BWD_CHILD " + json.dumps(res))
 
 
-def line_bwd_probe(limit_s: int = 240):
+def line_bwd_probe(limit_s: int = 150):
     """The line backward (csrc/gspn_line_bwd.cu) is not in GSPN_IMPL_AUTO: it had not run on hardware when round 2 ended.
     The bench gives it one bounded chance in a CHILD process (its own CUDA context, a time limit): forced with
     GSPN_IMPL_LINE on the two aligned configs, gated on sampled images against the oracle, then timed.  Whatever happens
