@@ -265,10 +265,14 @@ line_fwd_kernel(const __grid_constant__ CUtensorMap mxv, const __grid_constant__
     uint64_t* const full = bars;                   // [2][NS]
     uint64_t* const empty = bars + 2 * NS;         // [2][NS]
     uint64_t* const tfree = bars + 4 * NS;         // [2]: transposition tile t is free again
-    uint64_t* const fullh = bars + 4 * NS + 2;     // [3] column stages (shared by L->R and R->L)
-    uint64_t* const emptyh = bars + 4 * NS + 5;    // [3]
-    uint64_t* const vdone = bars + 4 * NS + 8;     // every scan-line warp has left the row stages
-    uint32_t* const tm_slot = reinterpret_cast<uint32_t*>(bars + 4 * NS + 9);
+    // column stages: 3 slots shared by L->R and R->L.  A slot alternates between the directions, and an mbarrier wait
+    // by parity must see EVERY phase of its barrier (a waiter that skips one takes the phase before for the one it
+    // wants), so each direction has its own "full" barrier per slot: its k-th use of a slot is phase k there.  The
+    // producer alone waits on the "empty" barriers, and it sees every phase.
+    uint64_t* const fullh = bars + 4 * NS + 2;     // [2 directions][3 slots]
+    uint64_t* const emptyh = bars + 4 * NS + 8;    // [3 slots]
+    uint64_t* const vdone = bars + 4 * NS + 11;    // every scan-line warp has left the row stages
+    uint32_t* const tm_slot = reinterpret_cast<uint32_t*>(bars + 4 * NS + 12);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int subs = prm.cg / NC;
@@ -282,7 +286,8 @@ line_fwd_kernel(const __grid_constant__ CUtensorMap mxv, const __grid_constant__
     if (threadIdx.x == 0) {
         for (int i = 0; i < 2 * NS; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], NC); }
         mbar_init(&tfree[0], 1); mbar_init(&tfree[1], 1);
-        for (int i = 0; i < 3; ++i) { mbar_init(&fullh[i], 1); mbar_init(&emptyh[i], NC); }
+        for (int i = 0; i < 6; ++i) mbar_init(&fullh[i], 1);
+        for (int i = 0; i < 3; ++i) mbar_init(&emptyh[i], NC);
         mbar_init(vdone, 2 * NC);
         mbar_init_fence();
     }
@@ -358,7 +363,7 @@ line_fwd_kernel(const __grid_constant__ CUtensorMap mxv, const __grid_constant__
                 if (2 + dd != cur_dir) { cur_dir = 2 + dd; roles(cur_dir, 1); }
                 const int stg = n % 3;
                 if (n >= 3) mbar_wait(&emptyh[stg], ((n / 3) - 1) & 1);
-                uint64_t* fb = &fullh[stg];
+                uint64_t* fb = &fullh[dd * 3 + stg];
                 if (lane == 0) { if (LINE_EXP == 2) mbar_arrive(fb); else mbar_arrive_expect_tx(fb, tx); }
                 __syncwarp();
                 if (issue && LINE_EXP != 2) {
@@ -429,7 +434,7 @@ line_fwd_kernel(const __grid_constant__ CUtensorMap mxv, const __grid_constant__
             const int first = both ? (d == 0 ? Wh : W - Wh) : W;
             for (int blk = 0; blk < nblk_h; ++blk) {
                 const int n = both ? 2 * blk + d : blk, stg = n % 3;      // place in the shared ring of column stages
-                mbar_wait(&fullh[stg], (n / 3) & 1);
+                mbar_wait(&fullh[d * 3 + stg], (blk / 3) & 1);      // this direction's (blk / 3)-th use of the slot
                 unsigned char* sb = ring + (size_t)stg * hstage_bytes;
                 line_zero_edge_taps_h(sb, cx.pbh, H, lane);
                 if (LINE_EXP == 1 || LINE_EXP == 3) {}
@@ -509,7 +514,7 @@ static int line_fwd_run(const FwdArgs<ST>& a, cudaStream_t st) {
     prm.tm_cols = cols;
     prm.h0 = a.h0; prm.y = a.y;
     prm.x = a.x; prm.w3 = a.w3; prm.lam = a.lam; prm.u = a.u;
-    const size_t smem = (size_t)prm.ring_bytes + (size_t)NT * 32 * prm.pitch * 4 + (4 * kLineStages + 9) * 8 + 16;
+    const size_t smem = (size_t)prm.ring_bytes + (size_t)NT * 32 * prm.pitch * 4 + (4 * kLineStages + 12) * 8 + 16;
     if (smem > (size_t)kMaxSmemOptin) return GSPN_EUNSUPPORTED;
 
     const int D = sh.D();
