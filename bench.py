@@ -48,7 +48,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--workload", default="cfg5_1k")
     ap.add_argument("--dtype", default=None, help="f32|bf16 (default: the workload's last listed dtype)")
-    ap.add_argument("--impl", default="gspn", choices=["gspn", "reference", "naive", "flat", "tile", "chain", "pair", "plane", "line"])
+    ap.add_argument("--impl", default="gspn", choices=["gspn", "reference", "naive", "flat", "tile", "chain", "plane", "line"])
     ap.add_argument("--no-others", action="store_true", help="skip the forward-only timings of the other configs")
     ap.add_argument("--no-parity", action="store_true", help="skip the sampled oracle check of the timed outputs")
     ap.add_argument("--no-e2e", action="store_true")
@@ -446,7 +446,7 @@ def main():
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     impl = {"naive": gspn.IMPL_NAIVE, "flat": gspn.IMPL_FLAT, "tile": gspn.IMPL_FUSED, "chain": gspn.IMPL_CHAIN,
-            "pair": gspn.IMPL_PAIR, "plane": gspn.IMPL_PLANE, "line": gspn.IMPL_LINE}.get(args.impl, gspn.IMPL_AUTO)
+            "plane": gspn.IMPL_PLANE, "line": gspn.IMPL_LINE}.get(args.impl, gspn.IMPL_AUTO)
 
     base = gi.CONFIGS[args.workload]
     dtype = args.dtype or base.dtypes[-1]

@@ -71,7 +71,7 @@ enum { GSPN_OK = 0, GSPN_EINVAL = 1, GSPN_EUNSUPPORTED = 2, GSPN_EALIGN = 3,
 enum { GSPN_IMPL_AUTO = 0, GSPN_IMPL_NAIVE = 1, GSPN_IMPL_FUSED = 2 /* 16-byte-aligned tile kernel */,
        GSPN_IMPL_FLAT = 3 /* any-shape fused kernel */,
        GSPN_IMPL_CHAIN = 4 /* warp-per-chain kernels (gspn_chain_*.cu) */,
-       GSPN_IMPL_PAIR = 5 /* forward: warp per direction carrying all channels of a CTA (gspn_pair_fwd.cu) */,
+       GSPN_IMPL_PAIR = 5 /* removed in round 2 (an A/B variant nothing selected): GSPN_EUNSUPPORTED; the value stays reserved */,
        GSPN_IMPL_PLANE = 6 /* small planes, forward and backward: whole operand planes on chip, 4 directions at once
                               (gspn_pair_fwd.cu plane_fwd, gspn_plane_bwd.cu) */,
        GSPN_IMPL_LINE = 7 /* 16-byte-aligned rows: warp per (channel, direction) line, several positions per lane,

@@ -61,7 +61,8 @@ static int fwd_typed(const gspn_args_t* a) {
     } else if (a->impl == GSPN_IMPL_CHAIN) {
         rc = chain_fwd_launch<ST>(f, st, &li);
     } else if (a->impl == GSPN_IMPL_PAIR) {
-        rc = pair_fwd_launch<ST>(f, st, &li);
+        set_error("GSPN_IMPL_PAIR: the ring-staged pair kernel was removed in round 2 (nothing selected it)");
+        rc = GSPN_EUNSUPPORTED;
     } else if (a->impl == GSPN_IMPL_PLANE) {
         rc = plane_fwd_launch<ST>(f, st, &li);
     } else if (a->impl == GSPN_IMPL_LINE) {

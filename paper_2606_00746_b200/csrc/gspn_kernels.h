@@ -27,7 +27,6 @@ template <typename ST> int chain_fwd_launch(const FwdArgs<ST>& a, cudaStream_t s
 
 // pair kernel (gspn_pair_fwd.cu): one warp carries all channels of a CTA for one direction (shared taps, NC*P
 // independent recurrences per lane), the two opposite directions of an axis run at the same time and share Y.
-template <typename ST> int pair_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 // whole-plane variant of the same for small planes (max(H,W) <= 64 and two CTAs' planes per SM): no rings
 template <typename ST> int plane_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 

@@ -18,8 +18,8 @@ pytestmark = pytest.mark.gpu
 
 IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO]
 IMPL_IDS = ["naive", "auto"]
-FWD_IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO, gspn.IMPL_FLAT, gspn.IMPL_CHAIN, gspn.IMPL_PAIR, gspn.IMPL_PLANE, gspn.IMPL_LINE]
-FWD_IMPL_IDS = ["naive", "auto", "flat", "chain", "pair", "plane", "line"]
+FWD_IMPLS = [gspn.IMPL_NAIVE, gspn.IMPL_AUTO, gspn.IMPL_FLAT, gspn.IMPL_CHAIN, gspn.IMPL_PLANE, gspn.IMPL_LINE]
+FWD_IMPL_IDS = ["naive", "auto", "flat", "chain", "plane", "line"]
 
 # (B, C, H, W, G): degenerate lines, W in {1,2,3}, H != W, beyond one warp, ragged tails, cg in {1,C}
 SMALL_SHAPES = [
@@ -329,7 +329,7 @@ def test_auto_selects_fused_kernels_where_supported():
 
 
 def test_chain_kernels_random_shapes():
-    """Seeded sweep of the chain kernels and the pair forward kernel (forced) over random shapes, masks, dtypes, group sizes and
+    """Seeded sweep of the chain kernels and the whole-plane forward kernel (forced) over random shapes, masks, dtypes, group sizes and
     initial states: ragged tails, lines of 1..128 positions, 1/2/4 channels per group."""
     import random
     rnd = random.Random(2024)
@@ -342,7 +342,7 @@ def test_chain_kernels_random_shapes():
             H, W = min(H, 40), min(W, 40)
         mask = rnd.randint(1, 15); dt = rnd.choice(["f32", "bf16"]); h0 = rnd.random() < 0.4
         cfg = gi.small_config("rz", B, C, H, W, G, dir_mask=mask, seed=3000 + it, backward=True)
-        for check, impl in ((pu.check_fwd, gspn.IMPL_CHAIN), (pu.check_bwd, gspn.IMPL_CHAIN), (pu.check_fwd, gspn.IMPL_PAIR), (pu.check_fwd, gspn.IMPL_PLANE)):
+        for check, impl in ((pu.check_fwd, gspn.IMPL_CHAIN), (pu.check_bwd, gspn.IMPL_CHAIN), (pu.check_fwd, gspn.IMPL_PLANE)):
             try:
                 r = check(cfg, dt, impl=impl, with_h0=h0)
             except gspn.GspnError as ex:
