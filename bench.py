@@ -330,9 +330,11 @@ def time_config(gspn, torch, cfg, dtype, steps, warmup, world, impl, want_bwd, t
     return res, tensors, y, grads
 
 
-def time_e2e(gspn, torch, cfg, dtype, steps, warmup, world, want_bwd, tensors):
+def time_e2e(gspn, torch, cfg, dtype, steps, warmup, world, want_bwd, tensors, fused=False):
     """Same metric through the host-pointer C-ABI entry points: pinned host operands, H2D copies,
-    kernels and D2H copies of every output inside the timed region."""
+    kernels and D2H copies of every output inside the timed region.  fused: one gspn_scan_fwd_bwd_host per step
+    (operands uploaded once, batch chunks pipelined over three streams) instead of the forward call followed by the
+    backward call."""
     host = {k: v.cpu().pin_memory() for k, v in tensors.items()}
     y = torch.empty_like(host["x"]).pin_memory()
     outs = None
@@ -345,10 +347,14 @@ def time_e2e(gspn, torch, cfg, dtype, steps, warmup, world, want_bwd, tensors):
     h2d = sum(nb(host[k]) for k in ("x", "w3", "lam", "u"))
     d2h = nb(y)
     if want_bwd:
-        h2d += sum(nb(host[k]) for k in ("x", "w3", "lam", "u", "dy"))
+        h2d += sum(nb(host[k]) for k in (("dy",) if fused else ("x", "w3", "lam", "u", "dy")))
         d2h += sum(nb(v) for v in outs.values())
 
     def step():
+        if fused and want_bwd:
+            gspn.gspn_scan_fwd_bwd_host(host["x"], host["w3"], host["lam"], host["u"], host["dy"], y, outs["dx"],
+                                        outs["dlambda"], outs["du"], outs["dw3"], outs["dh0"], cfg.G, cfg.dir_mask)
+            return
         gspn.gspn_scan_fwd_host(host["x"], host["w3"], host["lam"], host["u"], y, cfg.G, cfg.dir_mask)
         if want_bwd:
             gspn.gspn_scan_bwd_host(host["x"], host["w3"], host["lam"], host["u"], host["dy"], outs["dx"],
@@ -496,17 +502,38 @@ def main():
 
     e2e = None
     if not args.no_e2e:
-        ms, h2d, d2h, ye, oute, n_e2e = time_e2e(gspn, torch, cfg, dtype, steps, warmup, world, want_bwd, tensors)
-        e2e = {"value": world * step_bytes / (ms * 1e-3) / 1e9, "unit": "GB/s", "ms_per_step": ms,
-               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e,
-               "api": "gspn_scan_fwd_host" + (" + gspn_scan_bwd_host" if want_bwd else "")}
-        if not args.no_parity and rank == 0:      # the host path's own outputs are gated too, not only the device path's
-            import parity_util as pu
-            pe = pu.check_fwd_sampled(cfg, dtype, tensors, ye)
-            e2e["parity"] = {"fwd_ok": pe["ok"]}
-            if want_bwd:
-                e2e["parity"]["bwd_ok"] = pu.check_bwd_sampled(cfg, dtype, tensors, oute)["ok"]
-        del ye, oute
+        import parity_util as pu
+
+        def e2e_leg(fused):
+            ms, h2d, d2h, ye, oute, n_e2e = time_e2e(gspn, torch, cfg, dtype, steps, warmup, world, want_bwd, tensors, fused)
+            leg = {"value": world * step_bytes / (ms * 1e-3) / 1e9, "unit": "GB/s", "ms_per_step": ms,
+                   "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": n_e2e,
+                   "api": "gspn_scan_fwd_bwd_host" if fused and want_bwd else
+                          "gspn_scan_fwd_host" + (" + gspn_scan_bwd_host" if want_bwd else "")}
+            ok = True
+            if not args.no_parity and rank == 0:   # the host path's own outputs are gated too, not only the device path's
+                leg["parity"] = {"fwd_ok": pu.check_fwd_sampled(cfg, dtype, tensors, ye)["ok"]}
+                if want_bwd:
+                    leg["parity"]["bwd_ok"] = pu.check_bwd_sampled(cfg, dtype, tensors, oute)["ok"]
+                ok = all(leg["parity"].values())
+            return leg, ok
+
+        # the fused, pipelined host call (r2) is the public end-to-end path for a training step; it was written after GPU
+        # access had closed, so the two-call path that round 1 measured is the fall-back if it errs or misses parity
+        e2e = None
+        if want_bwd and world == 1:
+            try:
+                leg, ok = e2e_leg(True)
+                if ok:
+                    e2e = leg
+                else:
+                    fused_note = {"fused_call": "outputs failed the parity gate: not used", "fused_leg": leg}
+            except Exception as ex:      # noqa: BLE001
+                fused_note = {"fused_call": "raised " + repr(ex)[:200]}
+        if e2e is None:
+            e2e, _ = e2e_leg(False)
+            if want_bwd and world == 1:
+                e2e.update(fused_note)
     del grads, y
 
     others = None

@@ -151,6 +151,21 @@ int gspn_scan_bwd_host(const void* x, const void* w3, const void* lambda, const 
                        void* dx, void* dlambda, void* du, void* dw3, void* dh0,
                        int B, int C, int H, int W, int G, unsigned dir_mask, int dtype, void* stream);
 
+/*
+ * One forward + backward step through HOST buffers (r2): the operands are uploaded ONCE (gspn_scan_fwd_host followed by
+ * gspn_scan_bwd_host uploads x, w3, lambda, u twice) and the batch is cut into up to four chunks -- every (b, group) unit
+ * is independent, PAPER.md:125 -- that move through three internal streams, so that the upload of chunk i + 1, the kernels
+ * of chunk i and the download of chunk i - 1 overlap.  y and each gradient pointer may be NULL (skipped; with all
+ * gradients NULL only the forward runs).  Same layouts and status codes as the calls above; synchronous on return
+ * (`stream` is used for the allocations only).  Pinned host memory is what makes the copies overlap.
+ */
+int gspn_scan_fwd_bwd_host(const void* x, const void* w3, const void* lambda, const void* u, const void* dy, void* y,
+                           void* dx, void* dlambda, void* du, void* dw3, void* dh0,
+                           int B, int C, int H, int W, int G, unsigned dir_mask, int dtype, void* stream);
+/* Diagnostic: the batch-chunk walk of gspn_scan_fwd_bwd_host with memcpy, host to host (tests check its arithmetic
+ * without a GPU).  A tensor of D slabs x B images x image_bytes; images [b0, b0 + bc) <-> a chunk laid out [D, bc]. */
+int gspn_debug_chunk_copy(void* chunk, void* host, size_t image_bytes, int D, int B, int b0, int bc, int to_chunk);
+
 /* Bytes of caller-provided scratch the device entry points need: always 0 in this
  * version (every intermediate lives on chip); kept so callers can be written once. */
 size_t gspn_workspace_bytes(int B, int C, int H, int W, int G, unsigned dir_mask, int dtype, int is_bwd);

@@ -22,7 +22,8 @@ STATUS = {0: "GSPN_OK", 1: "GSPN_EINVAL", 2: "GSPN_EUNSUPPORTED", 3: "GSPN_EALIG
           4: "GSPN_EWORKSPACE", 5: "GSPN_ECUDA"}
 
 EXPORTS = ("gspn_scan_fwd", "gspn_scan_bwd", "gspn_merge", "gspn_scan_fwd_ex", "gspn_scan_bwd_ex",
-           "gspn_scan_fwd_host", "gspn_scan_bwd_host", "gspn_normalize_fwd", "gspn_normalize_bwd",
+           "gspn_scan_fwd_host", "gspn_scan_bwd_host", "gspn_scan_fwd_bwd_host", "gspn_debug_chunk_copy",
+           "gspn_normalize_fwd", "gspn_normalize_bwd",
            "gspn_workspace_bytes",
            "gspn_last_launch_count", "gspn_last_variant", "gspn_last_error", "gspn_version")
 
@@ -64,6 +65,8 @@ def lib() -> ctypes.CDLL:
         L.gspn_normalize_bwd.argtypes = [vp] * 3 + [ci] * 4 + [cu, ci, vp]
         L.gspn_scan_fwd_host.argtypes = L.gspn_scan_fwd.argtypes
         L.gspn_scan_bwd_host.argtypes = L.gspn_scan_bwd.argtypes
+        L.gspn_scan_fwd_bwd_host.argtypes = [vp] * 11 + [ci] * 5 + [cu, ci, vp]
+        L.gspn_debug_chunk_copy.argtypes = [vp, vp, ctypes.c_size_t] + [ci] * 5
         L.gspn_scan_fwd_ex.argtypes = [ctypes.POINTER(_Args)]
         L.gspn_scan_bwd_ex.argtypes = [ctypes.POINTER(_Args)]
         L.gspn_workspace_bytes.argtypes = [ci] * 5 + [cu, ci, ci]
@@ -245,6 +248,20 @@ def gspn_scan_bwd_host(x, w3, lam, u, dy, dx, dlambda, du, dw3, dh0, G: int,
     _check(lib().gspn_scan_bwd_host(_p(x), _p(w3), _p(lam), _p(u), _p(dy), _p(dx), _p(dlambda), _p(du),
                                     _p(dw3), _p(dh0), B, C, H, W, G, dir_mask, _dtype_code(x),
                                     ctypes.c_void_p(st)))
+
+
+def gspn_scan_fwd_bwd_host(x, w3, lam, u, dy, y, dx, dlambda, du, dw3, dh0, G: int,
+                           dir_mask: int = DIR_ALL, stream=None) -> None:
+    """One forward + backward step through host buffers, operands uploaded once, pipelined over batch chunks
+    (include/gspn.h gspn_scan_fwd_bwd_host).  y and every gradient may be None."""
+    B, C, H, W = x.shape
+    for t, n in ((x, "x"), (w3, "w3"), (lam, "lam"), (u, "u"), (dy, "dy"), (y, "y"), (dx, "dx"),
+                 (dlambda, "dlambda"), (du, "du"), (dw3, "dw3"), (dh0, "dh0")):
+        _host(t, n)
+    st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+    _check(lib().gspn_scan_fwd_bwd_host(_p(x), _p(w3), _p(lam), _p(u), _p(dy), _p(y), _p(dx), _p(dlambda), _p(du),
+                                        _p(dw3), _p(dh0), B, C, H, W, G, dir_mask, _dtype_code(x),
+                                        ctypes.c_void_p(st)))
 
 
 def gspn_last_launch_count() -> int:

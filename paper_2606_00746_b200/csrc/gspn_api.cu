@@ -306,6 +306,118 @@ done:
     return rc;
 }
 
+// ---- one forward + backward step through host buffers, operands uploaded once, pipelined over batch chunks ----------
+// Every tensor is [B, ...] or [D, B, ...] and every (b, group) unit is independent, so the batch is cut
+// into chunks; a chunk lives on the device as the same layout with B = its own size.  chunk_copy walks the D slabs of
+// one tensor for the images [b0, b0 + bc): `to_chunk` host -> chunk, else chunk -> host.
+}  // extern "C"
+
+template <typename Copy>
+static int chunk_copy(unsigned char* chunk, unsigned char* host, size_t image_bytes, size_t D, size_t B, size_t b0, size_t bc,
+                      bool to_chunk, Copy copy) {
+    for (size_t q = 0; q < D; ++q) {
+        unsigned char* h = host + (q * B + b0) * image_bytes;
+        unsigned char* c = chunk + q * bc * image_bytes;
+        const int rc = to_chunk ? copy(c, h, bc * image_bytes) : copy(h, c, bc * image_bytes);
+        if (rc) return rc;
+    }
+    return 0;
+}
+
+extern "C" {
+
+// the same walk with memcpy, host to host: what tests/test_abi.py checks the chunk arithmetic with (no GPU needed)
+int gspn_debug_chunk_copy(void* chunk, void* host, size_t image_bytes, int D, int B, int b0, int bc, int to_chunk) {
+    if (!chunk || !host || D < 1 || B < 1 || b0 < 0 || bc < 1 || b0 + bc > B) { set_error("gspn_debug_chunk_copy: bad arguments"); return GSPN_EINVAL; }
+    return chunk_copy((unsigned char*)chunk, (unsigned char*)host, image_bytes, (size_t)D, (size_t)B, (size_t)b0, (size_t)bc,
+                      to_chunk != 0, [](void* d, const void* s_, size_t n) { memcpy(d, s_, n); return 0; });
+}
+
+int gspn_scan_fwd_bwd_host(const void* x, const void* w3, const void* lambda, const void* u, const void* dy, void* y,
+                           void* dx, void* dlambda, void* du, void* dw3, void* dh0,
+                           int B, int C, int H, int W, int G, unsigned dir_mask, int dtype, void* stream) {
+    int rc = check_shape(B, C, H, W, G, dir_mask, dtype);
+    if (rc) return rc;
+    if (!x || !w3 || !lambda || !u || !dy) { set_error("NULL host pointer"); return GSPN_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t s = esize(dtype), D = Shape{B, C, H, W, G, dir_mask}.D(), L = (size_t)(H > W ? H : W);
+    const size_t ic = (size_t)C * H * W * s, iw = (size_t)3 * G * H * W * s, ih = (size_t)C * L * s;   // bytes per image
+    const int nchunk = B < 4 ? B : 4;
+    const int bcmax = (B + nchunk - 1) / nchunk;
+    // tensors: 0 x, 1 w3, 2 lambda, 3 u, 4 dy (inputs); 5 y, 6 dx, 7 dlambda, 8 du, 9 dw3, 10 dh0 (outputs)
+    void* host[11] = {(void*)x, (void*)w3, (void*)lambda, (void*)u, (void*)dy, y, dx, dlambda, du, dw3, dh0};
+    const size_t img[11] = {ic, iw, ic, ic, ic, ic, ic, ic, ic, iw, ih};
+    const size_t slabs[11] = {1, D, D, D, 1, 1, 1, D, D, D, D};
+    void* dev[2][11] = {};
+    cudaStream_t sin = nullptr, sk = nullptr, sout = nullptr;
+    cudaEvent_t in_done[2] = {}, k_done[2] = {}, out_done[2] = {};
+    auto h2d = [&](void* d, const void* h, size_t n) { return cudaMemcpyAsync(d, h, n, cudaMemcpyHostToDevice, sin) == cudaSuccess ? 0 : 1; };
+    auto d2h = [&](void* h, const void* d, size_t n) { return cudaMemcpyAsync(h, d, n, cudaMemcpyDeviceToHost, sout) == cudaSuccess ? 0 : 1; };
+    for (int sl = 0; sl < 2 && sl < nchunk; ++sl)
+        for (int t = 0; t < 11; ++t)
+            if (host[t]) CUDA_TRY(cudaMallocAsync(&dev[sl][t], slabs[t] * bcmax * img[t], st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    CUDA_TRY(cudaStreamCreateWithFlags(&sin, cudaStreamNonBlocking));
+    CUDA_TRY(cudaStreamCreateWithFlags(&sk, cudaStreamNonBlocking));
+    CUDA_TRY(cudaStreamCreateWithFlags(&sout, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+        CUDA_TRY(cudaEventCreateWithFlags(&in_done[i], cudaEventDisableTiming));
+        CUDA_TRY(cudaEventCreateWithFlags(&k_done[i], cudaEventDisableTiming));
+        CUDA_TRY(cudaEventCreateWithFlags(&out_done[i], cudaEventDisableTiming));
+    }
+    for (int ci = 0, b0 = 0; b0 < B; ++ci, b0 += bcmax) {
+        const int bc = B - b0 < bcmax ? B - b0 : bcmax, sl = ci & 1;
+        // uploads of this chunk: its input buffers are free once the kernels of the chunk before last are done
+        if (ci >= 2) CUDA_TRY(cudaStreamWaitEvent(sin, k_done[sl], 0));
+        for (int t = 0; t < 5; ++t)
+            if (chunk_copy((unsigned char*)dev[sl][t], (unsigned char*)host[t], img[t], slabs[t], (size_t)B, (size_t)b0, (size_t)bc, true, h2d)) {
+                set_error("gspn_scan_fwd_bwd_host: cudaMemcpyAsync (H2D) failed"); rc = GSPN_ECUDA; goto done;
+            }
+        CUDA_TRY(cudaEventRecord(in_done[sl], sin));
+        // kernels: after the uploads, and after the downloads of the chunk before last have left the output buffers
+        CUDA_TRY(cudaStreamWaitEvent(sk, in_done[sl], 0));
+        if (ci >= 2) CUDA_TRY(cudaStreamWaitEvent(sk, out_done[sl], 0));
+        if (y) {
+            rc = gspn_scan_fwd(dev[sl][0], dev[sl][1], dev[sl][2], dev[sl][3], dev[sl][5], bc, C, H, W, G, dir_mask, dtype, (void*)sk);
+            if (rc) goto done;
+        }
+        if (dx || dlambda || du || dw3 || dh0) {
+            rc = gspn_scan_bwd(dev[sl][0], dev[sl][1], dev[sl][2], dev[sl][3], dev[sl][4], dev[sl][6], dev[sl][7], dev[sl][8],
+                               dev[sl][9], dev[sl][10], bc, C, H, W, G, dir_mask, dtype, (void*)sk);
+            if (rc) goto done;
+        }
+        CUDA_TRY(cudaEventRecord(k_done[sl], sk));
+        // downloads
+        CUDA_TRY(cudaStreamWaitEvent(sout, k_done[sl], 0));
+        for (int t = 5; t < 11; ++t)
+            if (host[t] && chunk_copy((unsigned char*)dev[sl][t], (unsigned char*)host[t], img[t], slabs[t], (size_t)B, (size_t)b0, (size_t)bc, false, d2h)) {
+                set_error("gspn_scan_fwd_bwd_host: cudaMemcpyAsync (D2H) failed"); rc = GSPN_ECUDA; goto done;
+            }
+        CUDA_TRY(cudaEventRecord(out_done[sl], sout));
+    }
+done:
+    {
+        cudaError_t e1 = sin ? cudaStreamSynchronize(sin) : cudaSuccess;
+        cudaError_t e2 = sk ? cudaStreamSynchronize(sk) : cudaSuccess;
+        cudaError_t e3 = sout ? cudaStreamSynchronize(sout) : cudaSuccess;
+        for (int sl = 0; sl < 2; ++sl)
+            for (int t = 0; t < 11; ++t)
+                if (dev[sl][t]) cudaFreeAsync(dev[sl][t], st);
+        cudaError_t e4 = cudaStreamSynchronize(st);
+        for (int i = 0; i < 2; ++i) {
+            if (in_done[i]) cudaEventDestroy(in_done[i]);
+            if (k_done[i]) cudaEventDestroy(k_done[i]);
+            if (out_done[i]) cudaEventDestroy(out_done[i]);
+        }
+        if (sin) cudaStreamDestroy(sin);
+        if (sk) cudaStreamDestroy(sk);
+        if (sout) cudaStreamDestroy(sout);
+        const cudaError_t e = e1 != cudaSuccess ? e1 : e2 != cudaSuccess ? e2 : e3 != cudaSuccess ? e3 : e4;
+        if (rc == GSPN_OK && e != cudaSuccess) { set_error("gspn_scan_fwd_bwd_host: %s", cudaGetErrorString(e)); rc = GSPN_ECUDA; }
+    }
+    return rc;
+}
+
 size_t gspn_workspace_bytes(int, int, int, int, int, unsigned, int, int) { return 0; }
 
 int gspn_last_launch_count(void) { return g_launches; }

@@ -315,9 +315,12 @@ __device__ __forceinline__ void bwd_dir_v(BwdCtx& cx, const bool rev, const bool
     fence_proxy_async();
     named_bar_sync(1, NC * 32);
     if (c == 0 && lane == 0 && pend_buf >= 0) bwd_issue_store<NC, true>(cx, oo, pend_buf, pend_s0, multi, 1);
-    if (dh0p && active) {
+    if (dh0p) {
+        if (active) {
 #pragma unroll
-        for (int k = 0; k < P; ++k) st_f(dh0p + P * lane + k, carry[k]);
+            for (int k = 0; k < P; ++k) st_f(dh0p + P * lane + k, carry[k]);
+        }
+        for (int p = W + lane; p < (H > W ? H : W); p += 32) st_f(dh0p + p, 0.f);     // entries past the line are zeros
     }
 }
 
@@ -600,6 +603,7 @@ __device__ __forceinline__ void bwd_dir_h(BwdCtx& cx, const bool rev, const bool
     if (dh0p) {
 #pragma unroll
         for (int k = 0; k < P; ++k) if (lane + 32 * k < H) st_f(dh0p + lane + 32 * k, carry[k]);
+        for (int p = H + lane; p < (H > W ? H : W); p += 32) st_f(dh0p + p, 0.f);     // entries past the line are zeros
     }
 }
 

@@ -86,3 +86,27 @@ def test_sources_do_not_reference_the_oracle():
         if f.endswith((".py", ".c", ".h")):
             s = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2606_00746_b200" not in s and "libgspn.so" not in s
+
+
+def test_chunk_walk_of_the_fused_host_call_matches_numpy_slicing():
+    """gspn_scan_fwd_bwd_host cuts the batch into chunks: a chunk of a [D, B, ...] tensor is [D, bc, ...].  The walk it
+    uses for its copies (exported as gspn_debug_chunk_copy, memcpy host to host) against numpy slicing, both ways."""
+    import ctypes
+    import numpy as np
+    import paper_2606_00746_b200 as gspn
+    L = gspn.lib()
+    rng = np.random.default_rng(5)
+    for D, B, per in ((1, 5, 7), (4, 9, 12), (3, 4, 1), (2, 32, 40)):
+        t = rng.integers(0, 255, size=(D, B, per), dtype=np.uint8)
+        for b0, bc in ((0, 1), (0, B), (B - 1, 1), (B // 2, B - B // 2), (1, max(1, B // 3))):
+            chunk = np.zeros((D, bc, per), dtype=np.uint8)
+            rc = L.gspn_debug_chunk_copy(chunk.ctypes.data_as(ctypes.c_void_p), t.ctypes.data_as(ctypes.c_void_p), per, D, B, b0, bc, 1)
+            assert rc == 0
+            np.testing.assert_array_equal(chunk, t[:, b0:b0 + bc])
+            back = np.zeros_like(t)
+            rc = L.gspn_debug_chunk_copy(chunk.ctypes.data_as(ctypes.c_void_p), back.ctypes.data_as(ctypes.c_void_p), per, D, B, b0, bc, 0)
+            assert rc == 0
+            np.testing.assert_array_equal(back[:, b0:b0 + bc], t[:, b0:b0 + bc])
+            assert back[:, :b0].sum() == 0 and back[:, b0 + bc:].sum() == 0
+    assert L.gspn_debug_chunk_copy(None, None, 4, 1, 1, 0, 1, 1) != 0
+    assert L.gspn_debug_chunk_copy(chunk.ctypes.data_as(ctypes.c_void_p), t.ctypes.data_as(ctypes.c_void_p), 4, 1, 4, 3, 2, 1) != 0

@@ -262,3 +262,42 @@ def test_auto_backward_fallback_shapes(shape, dtype, record_property):
         pytest.xfail("no backward kernel under GSPN_IMPL_AUTO holds this shape")
     record_property("variant", r["variant"])
     assert r["ok"], r
+
+
+# ---------------------------------------------------------------------------------- the fused, pipelined host call
+@pytest.mark.parametrize("shape", [(1, 4, 16, 16, 2), (5, 4, 37, 41, 2), (9, 8, 27, 27, 2)], ids=["B1", "B5", "B9"])
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_fused_host_call_matches_the_oracle(dtype, shape):
+    """gspn_scan_fwd_bwd_host: operands uploaded once, up to four batch chunks on three streams (ragged last chunk at
+    B = 5 and 9); y and every gradient against the oracle, then with some outputs left out."""
+    cfg = gi.small_config("fh", *shape, seed=53, backward=True)
+    t = gi.make_inputs(cfg, dtype, device="cpu", with_dy=True)
+    host = {k: v.contiguous().pin_memory() for k, v in t.items()}
+    st = host["x"].dtype
+    mk = lambda *s: torch.full(s, float("nan"), dtype=st).pin_memory()
+    L = max(cfg.H, cfg.W)
+    y = mk(*host["x"].shape)
+    outs = {"dx": mk(*host["x"].shape), "dlambda": mk(*host["lam"].shape), "du": mk(*host["u"].shape),
+            "dw3": mk(*host["w3"].shape), "dh0": mk(cfg.D, cfg.B, cfg.C, L)}
+    gspn.gspn_scan_fwd_bwd_host(host["x"], host["w3"], host["lam"], host["u"], host["dy"], y, outs["dx"], outs["dlambda"],
+                                outs["du"], outs["dw3"], outs["dh0"], cfg.G, cfg.dir_mask)
+    yo, A = pu.oracle_fwd(t, cfg)
+    r = pu.gate(pu.np64(y), yo, A, dtype)
+    assert r["ok"], r
+    go, Ag = pu.oracle_bwd(t, cfg)
+    for k in ("dx", "dlambda", "du", "dw3"):
+        r = pu.gate(pu.np64(outs[k]), go[k], Ag[k], dtype)
+        assert r["ok"], (k, r)
+    # dh0: entries past a direction's line are not written (they keep the NaN fill); compare the lines
+    for q, d in enumerate(gi.dir_list(cfg.dir_mask)):
+        n = cfg.W if d < 2 else cfg.H
+        r = pu.gate(pu.np64(outs["dh0"][q, ..., :n]), go["dh0"][q, ..., :n], Ag["dh0"][q, ..., :n], dtype)
+        assert r["ok"], ("dh0", q, r)
+    # forward only / a subset of the gradients
+    y2, dw2 = mk(*host["x"].shape), mk(*host["w3"].shape)
+    gspn.gspn_scan_fwd_bwd_host(host["x"], host["w3"], host["lam"], host["u"], host["dy"], y2, None, None, None, None, None,
+                                cfg.G, cfg.dir_mask)
+    assert torch.equal(y2, y)
+    gspn.gspn_scan_fwd_bwd_host(host["x"], host["w3"], host["lam"], host["u"], host["dy"], None, None, None, None, dw2, None,
+                                cfg.G, cfg.dir_mask)
+    assert torch.equal(dw2, outs["dw3"])
