@@ -385,9 +385,10 @@ __device__ __forceinline__ void bwd_zero_edge_taps_h(unsigned char* sb, uint32_t
     __syncwarp();
 }
 
-template <typename ST, int NC, int P>
-__device__ __forceinline__ void bwd_dir_h(BwdCtx& cx, const bool rev, const bool acc, const ST* h0p, ST* dh0p,
+template <typename ST, int NC, int P, bool REV>
+__device__ __forceinline__ void bwd_dir_h(BwdCtx& cx, const bool acc, const ST* h0p, ST* dh0p,
                                           const BwdOut& oo, int multi) {
+    constexpr bool rev = REV;          // compile-time: the element order inside a sub-piece indexes registers
     using PL = BwdPlanes<NC>;
     constexpr int S = kLineSteps, NS = kBwdStages, ES = sizeof(ST), K = 16 / ES;
     const int H = cx.H, W = cx.W, lane = cx.lane, c = cx.c;
@@ -733,7 +734,8 @@ line_bwd_kernel(const __grid_constant__ BwdMaps mv, const __grid_constant__ BwdM
             oo.pc = (q * prm.B + b) * prm.C + c0; oo.pw = ((q * prm.B + b) * prm.G + g) * 3;
             oo.want_dlam = prm.want_dlam; oo.want_du = prm.want_du; oo.want_dw3 = prm.want_dw3;
             if (dir < 2) bwd_dir_v<ST, NC, P>(cx, dir & 1, acc, h0p, dh0p, oo, prm.multi);
-            else bwd_dir_h<ST, NC, P>(cx, dir & 1, acc, h0p, dh0p, oo, prm.multi);
+            else if (dir & 1) bwd_dir_h<ST, NC, P, true>(cx, acc, h0p, dh0p, oo, prm.multi);
+            else bwd_dir_h<ST, NC, P, false>(cx, acc, h0p, dh0p, oo, prm.multi);
             acc = true;
         }
         // ---- dx leaves: one RNE per element
