@@ -138,7 +138,24 @@ typedef struct gspn_args {
     int dtype;
     int impl;                      /* GSPN_IMPL_* */
     void *stream;
+    /* r2 (reading 6; Eq. 7 writes the propagation operands without a direction index).
+     * ELEMENT stride between the direction slabs of the INPUTS w3 / lambda / u:
+     *     GSPN_DIR_STRIDE_DENSE, or the dense value itself (3*B*G*H*W for w3, B*C*H*W for lambda and u):
+     *         the [D, ...] layout above, one slab per direction -- what every plain call uses;
+     *     0:  ONE slab ([B,G,3,H,W] / [B,C,H,W]) read by every direction of dir_mask.  The operand's algorithmic
+     *         bytes drop from D slabs to one.
+     *     any other value: GSPN_EINVAL.
+     * A struct whose fields were zeroed therefore asks for SHARED slabs: set the three fields to GSPN_DIR_STRIDE_DENSE
+     * for the dense layout, or pass struct_size = GSPN_ARGS_SIZE_R1 (the struct up to `stream`), which means dense.
+     * Outputs are never shared: dlambda, du, dw3 (and h0 / dh0) keep one slab per direction; the gradient of a shared
+     * slab is the sum of its D per-direction slabs, in whatever order and precision the caller wants.
+     * Shared slabs are served by the naive kernels only in this version (GSPN_IMPL_AUTO or GSPN_IMPL_NAIVE; any other
+     * impl reports GSPN_EUNSUPPORTED), so the shapes are those the naive kernels hold. */
+    size_t dir_stride_w3, dir_stride_lambda, dir_stride_u;
 } gspn_args_t;
+
+#define GSPN_DIR_STRIDE_DENSE ((size_t)-1)
+#define GSPN_ARGS_SIZE_R1 (offsetof(gspn_args_t, dir_stride_w3))
 
 int gspn_scan_fwd_ex(const gspn_args_t* a);
 int gspn_scan_bwd_ex(const gspn_args_t* a);

@@ -43,7 +43,23 @@ class _Args(ctypes.Structure):
                 ("dw3", ctypes.c_void_p), ("dh0", ctypes.c_void_p),
                 ("B", ctypes.c_int), ("C", ctypes.c_int), ("H", ctypes.c_int), ("W", ctypes.c_int),
                 ("G", ctypes.c_int), ("dir_mask", ctypes.c_uint), ("dtype", ctypes.c_int),
-                ("impl", ctypes.c_int), ("stream", ctypes.c_void_p)]
+                ("impl", ctypes.c_int), ("stream", ctypes.c_void_p),
+                ("dir_stride_w3", ctypes.c_size_t), ("dir_stride_lambda", ctypes.c_size_t),
+                ("dir_stride_u", ctypes.c_size_t)]
+
+
+DIR_STRIDE_DENSE = ctypes.c_size_t(-1).value       # GSPN_DIR_STRIDE_DENSE
+SHAREABLE = ("w3", "lam", "u")
+
+
+def _strides(shared) -> dict:
+    """gspn_args_t.dir_stride_*: 0 for the operands named in `shared` (one slab read by every direction), else dense."""
+    bad = set(shared) - set(SHAREABLE)
+    if bad:
+        raise ValueError(f"shared: unknown operand(s) {sorted(bad)} (choose from {SHAREABLE})")
+    return {"dir_stride_w3": 0 if "w3" in shared else DIR_STRIDE_DENSE,
+            "dir_stride_lambda": 0 if "lam" in shared else DIR_STRIDE_DENSE,
+            "dir_stride_u": 0 if "u" in shared else DIR_STRIDE_DENSE}
 
 
 _lib = None
@@ -119,16 +135,19 @@ def _shapes(x, G, dir_mask):
 
 
 def gspn_scan_fwd(x, w3, lam, u, G: int, dir_mask: int = DIR_ALL, h0=None, out=None,
-                  impl: int = IMPL_AUTO):
-    """y = sum_d u_d * scan_d(x); see include/gspn.h gspn_scan_fwd / gspn_scan_fwd_ex."""
+                  impl: int = IMPL_AUTO, shared=()):
+    """y = sum_d u_d * scan_d(x); see include/gspn.h gspn_scan_fwd / gspn_scan_fwd_ex.
+    shared: operands among ("w3", "lam", "u") that hold ONE slab ([B,G,3,H,W] / [B,C,H,W], no D axis) read by every
+    direction (gspn_args_t.dir_stride_* = 0)."""
     if not x.is_cuda:
         raise ValueError("x: need a CUDA tensor (there is no CPU path)")
     B, C, H, W, D, s_bc, s_w, s_h0 = _shapes(x, G, dir_mask)
-    _dev(x, "x", x.shape, x); _dev(w3, "w3", s_w, x); _dev(lam, "lam", s_bc, x); _dev(u, "u", s_bc, x)
+    _dev(x, "x", x.shape, x); _dev(w3, "w3", s_w[1:] if "w3" in shared else s_w, x)
+    _dev(lam, "lam", s_bc[1:] if "lam" in shared else s_bc, x); _dev(u, "u", s_bc[1:] if "u" in shared else s_bc, x)
     _dev(h0, "h0", s_h0, x)
     y = torch.empty_like(x) if out is None else _dev(out, "out", x.shape, x)
     with torch.cuda.device(x.device):
-        if h0 is None and impl == IMPL_AUTO:
+        if h0 is None and impl == IMPL_AUTO and not shared:
             rc = lib().gspn_scan_fwd(_p(x), _p(w3), _p(lam), _p(u), _p(y), B, C, H, W, G, dir_mask,
                                      _dtype_code(x), _stream(x))
         else:
@@ -136,25 +155,27 @@ def gspn_scan_fwd(x, w3, lam, u, G: int, dir_mask: int = DIR_ALL, h0=None, out=N
                       lam=lam.data_ptr(), u=u.data_ptr(), h0=None if h0 is None else h0.data_ptr(),
                       y=y.data_ptr(), B=B, C=C, H=H, W=W, G=G, dir_mask=dir_mask,
                       dtype=_dtype_code(x), impl=impl,
-                      stream=torch.cuda.current_stream(x.device).cuda_stream)
+                      stream=torch.cuda.current_stream(x.device).cuda_stream, **_strides(shared))
             rc = lib().gspn_scan_fwd_ex(ctypes.byref(a))
     _check(rc)
     return y
 
 
 def gspn_scan_bwd(x, w3, lam, u, dy, G: int, dir_mask: int = DIR_ALL, h0=None,
-                  need=("dx", "dlambda", "du", "dw3", "dh0"), impl: int = IMPL_AUTO) -> dict:
-    """Adjoint of gspn_scan_fwd; returns the requested gradients (include/gspn.h gspn_scan_bwd)."""
+                  need=("dx", "dlambda", "du", "dw3", "dh0"), impl: int = IMPL_AUTO, shared=()) -> dict:
+    """Adjoint of gspn_scan_fwd; returns the requested gradients (include/gspn.h gspn_scan_bwd).
+    shared: as in gspn_scan_fwd; the gradients keep one slab per direction (the gradient of a shared slab is their sum)."""
     if not x.is_cuda:
         raise ValueError("x: need a CUDA tensor (there is no CPU path)")
     B, C, H, W, D, s_bc, s_w, s_h0 = _shapes(x, G, dir_mask)
-    _dev(x, "x", x.shape, x); _dev(w3, "w3", s_w, x); _dev(lam, "lam", s_bc, x); _dev(u, "u", s_bc, x)
+    _dev(x, "x", x.shape, x); _dev(w3, "w3", s_w[1:] if "w3" in shared else s_w, x)
+    _dev(lam, "lam", s_bc[1:] if "lam" in shared else s_bc, x); _dev(u, "u", s_bc[1:] if "u" in shared else s_bc, x)
     _dev(dy, "dy", x.shape, x); _dev(h0, "h0", s_h0, x)
     shapes = {"dx": x.shape, "dlambda": s_bc, "du": s_bc, "dw3": s_w, "dh0": s_h0}
     out = {k: torch.empty(shapes[k], dtype=x.dtype, device=x.device) for k in need}
     g = lambda k: out[k].data_ptr() if k in out else None
     with torch.cuda.device(x.device):
-        if h0 is None and impl == IMPL_AUTO:
+        if h0 is None and impl == IMPL_AUTO and not shared:
             rc = lib().gspn_scan_bwd(_p(x), _p(w3), _p(lam), _p(u), _p(dy), g("dx"), g("dlambda"),
                                      g("du"), g("dw3"), g("dh0"), B, C, H, W, G, dir_mask,
                                      _dtype_code(x), _stream(x))
@@ -164,7 +185,7 @@ def gspn_scan_bwd(x, w3, lam, u, dy, G: int, dir_mask: int = DIR_ALL, h0=None,
                       dy=dy.data_ptr(), dx=g("dx"), dlambda=g("dlambda"), du=g("du"), dw3=g("dw3"),
                       dh0=g("dh0"), B=B, C=C, H=H, W=W, G=G, dir_mask=dir_mask,
                       dtype=_dtype_code(x), impl=impl,
-                      stream=torch.cuda.current_stream(x.device).cuda_stream)
+                      stream=torch.cuda.current_stream(x.device).cuda_stream, **_strides(shared))
             rc = lib().gspn_scan_bwd_ex(ctypes.byref(a))
     _check(rc)
     return out

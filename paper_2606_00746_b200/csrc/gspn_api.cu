@@ -45,16 +45,29 @@ static int check_shape(int B, int C, int H, int W, int G, unsigned mask, int dty
         if ((p) && !aligned16(p)) { set_error("pointer '%s' is not 16-byte aligned", #p); return GSPN_EALIGN; } \
     } while (0)
 
+// gspn_args_t.dir_stride_*: which inputs have one slab shared by every direction (validated by check_ex)
+static unsigned shared_bits(const gspn_args_t* a) {
+    if (a->struct_size == GSPN_ARGS_SIZE_R1) return 0;
+    return (a->dir_stride_w3 == 0 ? kSharedW3 : 0u) | (a->dir_stride_lambda == 0 ? kSharedLam : 0u) |
+           (a->dir_stride_u == 0 ? kSharedU : 0u);
+}
+
 template <typename ST>
 static int fwd_typed(const gspn_args_t* a) {
     FwdArgs<ST> f;
     f.x = (const ST*)a->x; f.w3 = (const ST*)a->w3; f.lam = (const ST*)a->lambda;
     f.u = (const ST*)a->u; f.h0 = (const ST*)a->h0; f.y = (ST*)a->y;
-    f.sh = Shape{a->B, a->C, a->H, a->W, a->G, a->dir_mask};
+    f.sh = Shape{a->B, a->C, a->H, a->W, a->G, a->dir_mask, shared_bits(a)};
     cudaStream_t st = (cudaStream_t)a->stream;
     LaunchInfo li{0, ""};
     int rc;
-    if (a->impl == GSPN_IMPL_NAIVE) {
+    if (f.sh.shared) {      // one slab for every direction: the naive kernel only (include/gspn.h, dir_stride_*)
+        if (a->impl != GSPN_IMPL_AUTO && a->impl != GSPN_IMPL_NAIVE) {
+            set_error("shared direction slabs (dir_stride_* = 0) are served by the naive kernels only (impl %d asked)", a->impl);
+            return GSPN_EUNSUPPORTED;
+        }
+        rc = naive_fwd_launch<ST>(f, st, &li);
+    } else if (a->impl == GSPN_IMPL_NAIVE) {
         rc = naive_fwd_launch<ST>(f, st, &li);
     } else if (a->impl == GSPN_IMPL_FLAT) {
         rc = flat_fwd_launch<ST>(f, st, &li);
@@ -89,11 +102,17 @@ static int bwd_typed(const gspn_args_t* a) {
     f.u = (const ST*)a->u; f.h0 = (const ST*)a->h0; f.dy = (const ST*)a->dy;
     f.dx = (ST*)a->dx; f.dlam = (ST*)a->dlambda; f.du = (ST*)a->du; f.dw3 = (ST*)a->dw3;
     f.dh0 = (ST*)a->dh0;
-    f.sh = Shape{a->B, a->C, a->H, a->W, a->G, a->dir_mask};
+    f.sh = Shape{a->B, a->C, a->H, a->W, a->G, a->dir_mask, shared_bits(a)};
     cudaStream_t st = (cudaStream_t)a->stream;
     LaunchInfo li{0, ""};
     int rc;
-    if (a->impl == GSPN_IMPL_NAIVE) {
+    if (f.sh.shared) {
+        if (a->impl != GSPN_IMPL_AUTO && a->impl != GSPN_IMPL_NAIVE) {
+            set_error("shared direction slabs (dir_stride_* = 0) are served by the naive kernels only (impl %d asked)", a->impl);
+            return GSPN_EUNSUPPORTED;
+        }
+        rc = naive_bwd_launch<ST>(f, st, &li);
+    } else if (a->impl == GSPN_IMPL_NAIVE) {
         rc = naive_bwd_launch<ST>(f, st, &li);
     } else if (a->impl == GSPN_IMPL_FUSED) {
         rc = fused_bwd_launch<ST>(f, st, &li);
@@ -121,15 +140,30 @@ static int bwd_typed(const gspn_args_t* a) {
 
 static int check_ex(const gspn_args_t* a) {
     if (!a) { set_error("args is NULL"); return GSPN_EINVAL; }
-    if (a->struct_size != sizeof(gspn_args_t)) {
-        set_error("gspn_args_t.struct_size=%zu, expected %zu", a->struct_size, sizeof(gspn_args_t));
+    if (a->struct_size != sizeof(gspn_args_t) && a->struct_size != GSPN_ARGS_SIZE_R1) {
+        set_error("gspn_args_t.struct_size=%zu, expected %zu (or %zu, the round-1 layout without dir_stride_*)", a->struct_size,
+                  sizeof(gspn_args_t), (size_t)GSPN_ARGS_SIZE_R1);
         return GSPN_EINVAL;
     }
     if (a->impl < GSPN_IMPL_AUTO || a->impl > GSPN_IMPL_LINE) {
         set_error("unknown impl %d", a->impl);
         return GSPN_EINVAL;
     }
-    return check_shape(a->B, a->C, a->H, a->W, a->G, a->dir_mask, a->dtype);
+    int rc = check_shape(a->B, a->C, a->H, a->W, a->G, a->dir_mask, a->dtype);
+    if (rc) return rc;
+    if (a->struct_size == sizeof(gspn_args_t)) {
+        const size_t hw = (size_t)a->H * a->W;
+        const size_t dense[3] = {(size_t)3 * a->B * a->G * hw, (size_t)a->B * a->C * hw, (size_t)a->B * a->C * hw};
+        const size_t got[3] = {a->dir_stride_w3, a->dir_stride_lambda, a->dir_stride_u};
+        const char* name[3] = {"dir_stride_w3", "dir_stride_lambda", "dir_stride_u"};
+        for (int t = 0; t < 3; ++t)
+            if (got[t] != 0 && got[t] != GSPN_DIR_STRIDE_DENSE && got[t] != dense[t]) {
+                set_error("%s=%zu: only 0 (one slab shared by every direction) and the dense stride %zu (GSPN_DIR_STRIDE_DENSE) "
+                          "are supported", name[t], got[t], dense[t]);
+                return GSPN_EINVAL;
+            }
+    }
+    return GSPN_OK;
 }
 
 static size_t esize(int dtype) { return dtype == GSPN_F32 ? 4 : 2; }
@@ -166,6 +200,7 @@ int gspn_scan_fwd(const void* x, const void* w3, const void* lambda, const void*
     a.x = x; a.w3 = w3; a.lambda = lambda; a.u = u; a.y = y;
     a.B = B; a.C = C; a.H = H; a.W = W; a.G = G; a.dir_mask = dir_mask; a.dtype = dtype;
     a.impl = GSPN_IMPL_AUTO; a.stream = stream;
+    a.dir_stride_w3 = a.dir_stride_lambda = a.dir_stride_u = GSPN_DIR_STRIDE_DENSE;
     return gspn_scan_fwd_ex(&a);
 }
 
@@ -179,6 +214,7 @@ int gspn_scan_bwd(const void* x, const void* w3, const void* lambda, const void*
     a.dx = dx; a.dlambda = dlambda; a.du = du; a.dw3 = dw3; a.dh0 = dh0;
     a.B = B; a.C = C; a.H = H; a.W = W; a.G = G; a.dir_mask = dir_mask; a.dtype = dtype;
     a.impl = GSPN_IMPL_AUTO; a.stream = stream;
+    a.dir_stride_w3 = a.dir_stride_lambda = a.dir_stride_u = GSPN_DIR_STRIDE_DENSE;
     return gspn_scan_bwd_ex(&a);
 }
 

@@ -28,9 +28,14 @@ __device__ __forceinline__ int img_off(int dir, int s, int p, int H, int W) {
     }
 }
 
+constexpr unsigned kSharedW3 = 1u, kSharedLam = 2u, kSharedU = 4u;
+
 struct Shape {
     int B, C, H, W, G;
     unsigned mask;
+    // operands whose direction slabs are ONE slab read by every direction (gspn_args_t.dir_stride_* == 0, DESIGN.md
+    // reading 6): bits kSharedW3 / kSharedLam / kSharedU.  0 = the dense [D, ...] layout.  Outputs are never shared.
+    unsigned shared;
     __host__ __device__ int cg() const { return C / G; }
     __host__ __device__ int Lmax() const { return H > W ? H : W; }
     __host__ __device__ size_t plane() const { return (size_t)H * W; }

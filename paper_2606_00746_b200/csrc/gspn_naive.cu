@@ -65,6 +65,18 @@ __device__ void naive_pass_fwd(int dir, const ST* xp, const ST* wp, const ST* lp
     }
 }
 
+// plane index of the INPUT operands of direction slab q: a shared operand (Shape::shared) has one slab, read by every
+// direction; h0 and every output keep one slab per direction
+struct SlabIn {
+    size_t w, l, u;       // w3 plane triple, lambda plane, u plane
+    __device__ SlabIn(const Shape& sh, int q, int b, int c, int g) {
+        const size_t qw = sh.shared & kSharedW3 ? 0 : q, ql = sh.shared & kSharedLam ? 0 : q, qu = sh.shared & kSharedU ? 0 : q;
+        w = (qw * sh.B + b) * sh.G + g;
+        l = (ql * sh.B + b) * sh.C + c;
+        u = (qu * sh.B + b) * sh.C + c;
+    }
+};
+
 template <typename ST>
 __global__ void naive_fwd_kernel(FwdArgs<ST> a) {
     extern __shared__ float smem[];
@@ -79,9 +91,9 @@ __global__ void naive_fwd_kernel(FwdArgs<ST> a) {
     for (int dir = 0; dir < 4; ++dir) {
         if (!(sh.mask >> dir & 1)) continue;
         const size_t dbc = ((size_t)q * sh.B + b) * sh.C + c;
-        const size_t dbg = ((size_t)q * sh.B + b) * sh.G + g;
-        naive_pass_fwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + dbg * 3 * plane,
-                           a.lam + dbc * plane, a.u + dbc * plane,
+        const SlabIn in(sh, q, b, c, g);
+        naive_pass_fwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + in.w * 3 * plane,
+                           a.lam + in.l * plane, a.u + in.u * plane,
                            a.h0 ? a.h0 + dbc * Lmax : nullptr, hbuf, nullptr, ysm, H, W);
         ++q;
     }
@@ -181,12 +193,12 @@ __global__ void naive_bwd_main_kernel(BwdArgs<ST> a) {
     for (int dir = 0; dir < 4; ++dir) {
         if (!(sh.mask >> dir & 1)) continue;
         const size_t dbc = ((size_t)q * sh.B + b) * sh.C + c;
-        const size_t dbg = ((size_t)q * sh.B + b) * sh.G + g;
+        const SlabIn in(sh, q, b, c, g);
         const ST* h0p = a.h0 ? a.h0 + dbc * Lmax : nullptr;
-        naive_pass_fwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + dbg * 3 * plane,
-                           a.lam + dbc * plane, a.u + dbc * plane, h0p, hbuf, hall, nullptr, H, W);
-        naive_pass_bwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + dbg * 3 * plane,
-                           a.lam + dbc * plane, a.u + dbc * plane, h0p, a.dy + (size_t)bc * plane,
+        naive_pass_fwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + in.w * 3 * plane,
+                           a.lam + in.l * plane, a.u + in.u * plane, h0p, hbuf, hall, nullptr, H, W);
+        naive_pass_bwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + in.w * 3 * plane,
+                           a.lam + in.l * plane, a.u + in.u * plane, h0p, a.dy + (size_t)bc * plane,
                            hall, ghs, a.dx ? dxs : nullptr, nullptr,
                            a.dlam ? a.dlam + dbc * plane : nullptr,
                            a.du ? a.du + dbc * plane : nullptr,
@@ -222,11 +234,12 @@ __global__ void naive_bwd_dw_kernel(BwdArgs<ST> a) {
         const int c = g * cg + cc;
         const size_t bc = (size_t)b * sh.C + c;
         const size_t dbc = ((size_t)q * sh.B + b) * sh.C + c;
+        const SlabIn in(sh, q, b, c, g);
         const ST* h0p = a.h0 ? a.h0 + dbc * Lmax : nullptr;
-        naive_pass_fwd<ST>(dir, a.x + bc * plane, a.w3 + dbg * 3 * plane, a.lam + dbc * plane,
-                           a.u + dbc * plane, h0p, hbuf, hall, nullptr, H, W);
-        naive_pass_bwd<ST>(dir, a.x + bc * plane, a.w3 + dbg * 3 * plane, a.lam + dbc * plane,
-                           a.u + dbc * plane, h0p, a.dy + bc * plane, hall, ghs, nullptr, dws,
+        naive_pass_fwd<ST>(dir, a.x + bc * plane, a.w3 + in.w * 3 * plane, a.lam + in.l * plane,
+                           a.u + in.u * plane, h0p, hbuf, hall, nullptr, H, W);
+        naive_pass_bwd<ST>(dir, a.x + bc * plane, a.w3 + in.w * 3 * plane, a.lam + in.l * plane,
+                           a.u + in.u * plane, h0p, a.dy + bc * plane, hall, ghs, nullptr, dws,
                            nullptr, nullptr, nullptr, H, W);
         __syncthreads();
     }

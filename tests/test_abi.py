@@ -110,3 +110,35 @@ def test_chunk_walk_of_the_fused_host_call_matches_numpy_slicing():
             assert back[:, :b0].sum() == 0 and back[:, b0 + bc:].sum() == 0
     assert L.gspn_debug_chunk_copy(None, None, 4, 1, 1, 0, 1, 1) != 0
     assert L.gspn_debug_chunk_copy(chunk.ctypes.data_as(ctypes.c_void_p), t.ctypes.data_as(ctypes.c_void_p), 4, 1, 4, 3, 2, 1) != 0
+
+
+def test_dir_stride_fields_are_validated_without_gpu(L):
+    """gspn_args_t.dir_stride_* (include/gspn.h, reading 6): 0 = one slab shared by every direction,
+    GSPN_DIR_STRIDE_DENSE or the dense element count = one slab per direction, anything else GSPN_EINVAL; the round-1
+    struct (without the fields) is still accepted.  A backward call that asks for no output validates and returns."""
+    from paper_2606_00746_b200 import binding as bd
+    buf = ctypes.create_string_buffer(4096 + 16)
+    p = (ctypes.addressof(buf) + 15) & ~15
+    B, C, H, W, G = 2, 4, 5, 6, 2
+
+    def call(size=None, **kw):
+        a = bd._Args(struct_size=ctypes.sizeof(bd._Args) if size is None else size, x=p, w3=p, lam=p, u=p, dy=p,
+                     B=B, C=C, H=H, W=W, G=G, dir_mask=15, dtype=0, impl=0,
+                     dir_stride_w3=bd.DIR_STRIDE_DENSE, dir_stride_lambda=bd.DIR_STRIDE_DENSE, dir_stride_u=bd.DIR_STRIDE_DENSE)
+        for k, v in kw.items():
+            setattr(a, k, v)
+        return L.gspn_scan_bwd_ex(ctypes.byref(a))
+
+    assert call() == 0
+    assert call(dir_stride_w3=0) == 0 and call(dir_stride_lambda=0, dir_stride_u=0) == 0
+    assert call(dir_stride_w3=3 * B * G * H * W, dir_stride_lambda=B * C * H * W, dir_stride_u=B * C * H * W) == 0
+    assert call(dir_stride_w3=B * C * H * W) == 1 and b"dir_stride_w3" in L.gspn_last_error()
+    assert call(dir_stride_u=7) == 1 and b"dir_stride_u" in L.gspn_last_error()
+    r1 = bd._Args.dir_stride_w3.offset                      # GSPN_ARGS_SIZE_R1: the struct up to `stream`
+    assert r1 == bd._Args.stream.offset + ctypes.sizeof(ctypes.c_void_p)
+    assert call(size=r1, dir_stride_w3=12345) == 0          # fields beyond struct_size are not read
+    assert call(size=r1 + 8) == 1 and b"struct_size" in L.gspn_last_error()
+    # the binding's helper: names -> strides
+    assert bd._strides(("w3",)) == {"dir_stride_w3": 0, "dir_stride_lambda": bd.DIR_STRIDE_DENSE, "dir_stride_u": bd.DIR_STRIDE_DENSE}
+    with pytest.raises(ValueError):
+        bd._strides(("x",))

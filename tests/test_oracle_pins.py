@@ -648,3 +648,34 @@ def test_float_build_of_backward_tracks_double_build():
     for k in ("dx", "dlambda", "du", "dw3", "dh0"):
         assert g32[k].dtype == np.float32
         assert np.all(np.abs(g32[k] - g64[k]) <= np.maximum(1e-5 * A[k], 1e-6)), k
+
+
+@pytest.mark.parametrize("mask", [15, 6, 9])
+def test_out_of_grid_taps_are_never_read_by_the_oracle(mask):
+    """DESIGN.md reading 3 / include/gspn.h: the tap of a neighbour outside the grid is never used.  What a slab
+    SHARED by every direction (gspn_args_t.dir_stride_* = 0, reading 6) relies on: a tap that is in the grid for a
+    vertical scan lies outside it for a horizontal one and must then count as absent, whatever it holds.  NaN in every
+    out-of-grid tap changes no output; the dw3 entries of those taps are exactly 0."""
+    rng = np.random.default_rng(77)
+    B, C, H, W, G = 2, 4, 6, 9, 2
+    x, w3, lam, u = rand_problem(rng, B, C, H, W, G, mask)
+    dy = rng.standard_normal(x.shape)
+    bad = w3.copy()
+    out = np.zeros(w3.shape, bool)
+    for q, d in enumerate(dd for dd in range(4) if mask >> dd & 1):
+        if d < 2:
+            out[q, :, :, 0, :, 0] = True; out[q, :, :, 2, :, W - 1] = True
+        else:
+            out[q, :, :, 0, 0, :] = True; out[q, :, :, 2, H - 1, :] = True
+    bad[out] = np.nan
+    np.testing.assert_array_equal(orc.fwd(x, bad, lam, u, G, mask), orc.fwd(x, w3, lam, u, G, mask))
+    g0, g1 = orc.bwd(x, w3, lam, u, dy, G, mask), orc.bwd(x, bad, lam, u, dy, G, mask)
+    for k in g0:
+        np.testing.assert_array_equal(g1[k], g0[k], err_msg=k)
+    assert np.all(g1["dw3"][out] == 0.0)
+    # one slab replicated over the directions: its in-grid taps for one axis are out-of-grid taps for the other, so the
+    # result equals the one with those taps zeroed per direction
+    D = orc.popcount(mask)
+    rep = np.repeat(w3[:1], D, axis=0)
+    zeroed = rep.copy(); zeroed[out] = 0.0
+    np.testing.assert_array_equal(orc.fwd(x, rep, lam, u, G, mask), orc.fwd(x, zeroed, lam, u, G, mask))

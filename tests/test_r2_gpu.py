@@ -301,3 +301,42 @@ def test_fused_host_call_matches_the_oracle(dtype, shape):
     gspn.gspn_scan_fwd_bwd_host(host["x"], host["w3"], host["lam"], host["u"], host["dy"], None, None, None, None, dw2, None,
                                 cfg.G, cfg.dir_mask)
     assert torch.equal(dw2, outs["dw3"])
+
+
+# ---------------------------------------------------------------------------------- shared direction slabs
+SHARED_SETS = [("w3",), ("lam", "u"), ("w3", "lam", "u")]
+
+
+@pytest.mark.parametrize("shared", SHARED_SETS, ids=["+".join(s) for s in SHARED_SETS])
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_shared_direction_slabs(dtype, shared):
+    """gspn_args_t.dir_stride_* = 0 (reading 6): ONE slab of w3 / lambda / u read by every
+    direction.  Oracle: the same slab replicated over the D directions (what "shared" means); the gradients stay per
+    direction.  Also bit-identical to the dense call on the replicated operands (same kernel, same arithmetic), and
+    refused by every kernel but the naive one."""
+    for shape, mask in [((2, 4, 16, 16, 2), 15), ((1, 4, 37, 41, 2), 15), ((2, 2, 27, 27, 1), 6), ((1, 2, 70, 33, 1), 9)]:
+        cfg = gi.small_config("shr", *shape, dir_mask=mask, seed=88, backward=True)
+        t = gi.make_inputs(cfg, dtype, device="cpu", with_dy=True)
+        rep = dict(t)
+        for k in shared:
+            rep[k] = t[k][:1].expand(cfg.D, *t[k].shape[1:]).contiguous()
+        d = {k: v.cuda() for k, v in rep.items()}
+        one = {k: (t[k][0].contiguous().cuda() if k in shared else d[k]) for k in ("w3", "lam", "u")}
+        y = gspn.gspn_scan_fwd(d["x"], one["w3"], one["lam"], one["u"], cfg.G, mask, shared=shared)
+        assert gspn.gspn_last_variant() == "naive_fwd"
+        yo, A = pu.oracle_fwd(rep, cfg)
+        r = pu.gate(pu.np64(y), yo, A, dtype)
+        assert r["ok"], (shape, mask, r)
+        assert torch.equal(y, gspn.gspn_scan_fwd(d["x"], d["w3"], d["lam"], d["u"], cfg.G, mask, impl=gspn.IMPL_NAIVE))
+        g = gspn.gspn_scan_bwd(d["x"], one["w3"], one["lam"], one["u"], d["dy"], cfg.G, mask, shared=shared)
+        assert gspn.gspn_last_variant() == "naive_bwd"
+        go, Ag = pu.oracle_bwd(rep, cfg)
+        gd = gspn.gspn_scan_bwd(d["x"], d["w3"], d["lam"], d["u"], d["dy"], cfg.G, mask, impl=gspn.IMPL_NAIVE)
+        for k in ("dx", "dlambda", "du", "dw3", "dh0"):
+            assert tuple(g[k].shape) == tuple(gd[k].shape), k          # one slab per direction, shared or not
+            r = pu.gate(pu.np64(g[k]), go[k], Ag[k], dtype)
+            assert r["ok"], (shape, mask, k, r)
+            assert torch.equal(g[k], gd[k]), (shape, mask, k)
+    with pytest.raises(gspn.GspnError) as ei:
+        gspn.gspn_scan_fwd(d["x"], one["w3"], one["lam"], one["u"], cfg.G, mask, shared=shared, impl=gspn.IMPL_CHAIN)
+    assert ei.value.status == 2
