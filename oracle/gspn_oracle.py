@@ -166,3 +166,83 @@ def bwd_magnitude(x, w3, lam, u, dy, G: int, mask: int, h0=None):
     a = [np.abs(np.asarray(t, dtype=np.float64)) for t in (x, w3, lam, u, dy)]
     return bwd(a[0], a[1], a[2], a[3], a[4], G, mask,
                None if h0 is None else np.abs(np.asarray(h0, dtype=np.float64)))
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Chunked scan (SURVEY.md 8(f) f3; PAPER.md:125,129 use `k_chunk` in the launch grid `(chunk, b, c)` and never define it).
+# Reading (DESIGN.md reading 10): the scan axis is cut, in IMAGE coordinates, into k_chunk bands of Lc = ceil(L / k_chunk)
+# lines (the last band may be shorter, and fewer than k_chunk bands exist when Lc * (k_chunk - 1) >= L); every band is an
+# independent scan on its sub-grid with a zero initial state.  Both directions of an axis share the bands.  h0 / dh0 belong
+# to the band that holds scan step 0 of the direction.  The definition is written out as such: slice, call the plain
+# oracle above (one direction at a time) on the sub-grid, put the pieces back.  y sums the directions in ascending order.
+def chunk_bands(L: int, k_chunk: int):
+    """[(first line, one past the last line)] of the bands of a scan axis of L lines."""
+    assert k_chunk >= 1
+    Lc = -(-L // k_chunk)
+    return [(a, min(a + Lc, L)) for a in range(0, L, Lc)]
+
+
+def _band_views(d, a, b):
+    """Index tuples of band [a, b) of direction d for [B,C,H,W] and for one direction slab [1,B,*,...,H,W]."""
+    img = (slice(None), slice(None), slice(a, b), slice(None)) if d < 2 else (slice(None), slice(None), slice(None), slice(a, b))
+    return img, (Ellipsis,) + img[2:]
+
+
+def _band_h0(h0, q, d, a, b, H, W, shape_bc):
+    """h0 of the sub-problem: the direction's h0 for the band holding scan step 0, else None."""
+    L = H if d < 2 else W
+    holds_step0 = (a == 0) if d in (0, 2) else (b == L)
+    if h0 is None or not holds_step0:
+        return None, holds_step0
+    Lp = W if d < 2 else H
+    Hb, Wb = (b - a, W) if d < 2 else (H, b - a)
+    sub = np.zeros((1,) + shape_bc + (max(Hb, Wb),), dtype=h0.dtype)
+    sub[0, ..., :Lp] = h0[q, ..., :Lp]
+    return sub, holds_step0
+
+
+def fwd_chunked(x, w3, lam, u, G: int, mask: int, k_chunk: int, h0=None):
+    """y of the chunked scan: per direction and band, the plain forward on the sub-grid."""
+    dt = np.float32 if x.dtype == np.float32 else np.float64
+    x, w3, lam, u, h0 = (_prep(a, dt) for a in (x, w3, lam, u, h0))
+    B, C, H, W, D = _check(x, w3, lam, u, G, mask, h0)
+    y = np.zeros_like(x)
+    for q, d in enumerate(dd for dd in range(4) if mask >> dd & 1):
+        for a, b in chunk_bands(H if d < 2 else W, k_chunk):
+            img, slab = _band_views(d, a, b)
+            h0b, _ = _band_h0(h0, q, d, a, b, H, W, (B, C))
+            y[img] += fwd(x[img], w3[q:q + 1][slab], lam[q:q + 1][slab], u[q:q + 1][slab], G, 1 << d, h0=h0b)
+    return y
+
+
+def bwd_chunked(x, w3, lam, u, dy, G: int, mask: int, k_chunk: int, h0=None):
+    """Adjoint of fwd_chunked: per direction and band, the plain backward on the sub-grid; dx sums the directions in
+    ascending order; dh0 comes from the band that holds scan step 0 (entries past the line are 0)."""
+    dt = np.float32 if x.dtype == np.float32 else np.float64
+    x, w3, lam, u, dy, h0 = (_prep(a, dt) for a in (x, w3, lam, u, dy, h0))
+    B, C, H, W, D = _check(x, w3, lam, u, G, mask, h0)
+    out = dict(dx=np.zeros_like(x), dlambda=np.zeros_like(lam), du=np.zeros_like(u), dw3=np.zeros_like(w3),
+               dh0=np.zeros((D, B, C, max(H, W)), dtype=dt))
+    for q, d in enumerate(dd for dd in range(4) if mask >> dd & 1):
+        Lp = W if d < 2 else H
+        for a, b in chunk_bands(H if d < 2 else W, k_chunk):
+            img, slab = _band_views(d, a, b)
+            h0b, holds_step0 = _band_h0(h0, q, d, a, b, H, W, (B, C))
+            g = bwd(x[img], w3[q:q + 1][slab], lam[q:q + 1][slab], u[q:q + 1][slab], dy[img], G, 1 << d, h0=h0b)
+            out["dx"][img] += g["dx"]
+            out["dlambda"][q:q + 1][slab] = g["dlambda"]
+            out["du"][q:q + 1][slab] = g["du"]
+            out["dw3"][q:q + 1][slab] = g["dw3"]
+            if holds_step0:
+                out["dh0"][q, ..., :Lp] = g["dh0"][0, ..., :Lp]
+    return out
+
+
+def fwd_chunked_magnitude(x, w3, lam, u, G: int, mask: int, k_chunk: int, h0=None):
+    a = [np.abs(np.asarray(t, dtype=np.float64)) for t in (x, w3, lam, u)]
+    return fwd_chunked(a[0], a[1], a[2], a[3], G, mask, k_chunk, None if h0 is None else np.abs(np.asarray(h0, dtype=np.float64)))
+
+
+def bwd_chunked_magnitude(x, w3, lam, u, dy, G: int, mask: int, k_chunk: int, h0=None):
+    a = [np.abs(np.asarray(t, dtype=np.float64)) for t in (x, w3, lam, u, dy)]
+    return bwd_chunked(a[0], a[1], a[2], a[3], a[4], G, mask, k_chunk, None if h0 is None else np.abs(np.asarray(h0, dtype=np.float64)))
