@@ -152,6 +152,13 @@ typedef struct gspn_args {
      * Shared slabs are served by the naive kernels only in this version (GSPN_IMPL_AUTO or GSPN_IMPL_NAIVE; any other
      * impl reports GSPN_EUNSUPPORTED), so the shapes are those the naive kernels hold. */
     size_t dir_stride_w3, dir_stride_lambda, dir_stride_u;
+    /* r2 (PAPER.md:125,129 name `k_chunk` in the launch grid and never define it; reading 10).
+     * Chunked scan: the scan axis of every direction is cut, in IMAGE coordinates, into bands of ceil(L / k_chunk) lines
+     * (L = H for the vertical directions, W for the horizontal ones; the last band may be shorter), and every band is an
+     * independent scan on its sub-grid with a zero initial state.  Both directions of an axis share the bands.  h0 / dh0
+     * belong to the band that holds the direction's scan step 0.  0 or 1 = the global scan; negative: GSPN_EINVAL.
+     * k_chunk > 1 is served by the naive kernels only in this version (as shared slabs above). */
+    int k_chunk;
 } gspn_args_t;
 
 #define GSPN_DIR_STRIDE_DENSE ((size_t)-1)

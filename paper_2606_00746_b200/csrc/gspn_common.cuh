@@ -36,6 +36,10 @@ struct Shape {
     // operands whose direction slabs are ONE slab read by every direction (gspn_args_t.dir_stride_* == 0, DESIGN.md
     // reading 6): bits kSharedW3 / kSharedLam / kSharedU.  0 = the dense [D, ...] layout.  Outputs are never shared.
     unsigned shared;
+    // chunked scan (gspn_args_t.k_chunk, reading 10): bands of ceil(L / k_chunk) lines of the scan axis in image
+    // coordinates, each an independent scan with a zero initial state.  0 or 1 = one band (the global scan).
+    int k_chunk;
+    __host__ __device__ int band(int Ls) const { const int k = k_chunk > 1 ? k_chunk : 1; return (Ls + k - 1) / k; }
     __host__ __device__ int cg() const { return C / G; }
     __host__ __device__ int Lmax() const { return H > W ? H : W; }
     __host__ __device__ size_t plane() const { return (size_t)H * W; }

@@ -16,9 +16,16 @@ namespace gspn {
 //   ysm  : NULL or [H*W] floats, y += u*h
 constexpr int kChunk = 8;      // scan steps whose operands a thread fetches together (one global latency per chunk)
 
+//   Lc   : lines per band of the scan axis (chunked scan, Shape::band; Lc = Ls is the global scan)
+// step s enters a band (the state of the line before counts as zero) when its line, in image coordinates, is a band's
+// first line for the ascending directions (0, 2) and a band's last line for the descending ones (1, 3)
+__device__ __forceinline__ bool band_entry(int dir, int s, int Ls, int Lc) {
+    return s > 0 && ((dir & 1) ? (Ls - 1 - s) % Lc == Lc - 1 : s % Lc == 0);
+}
+
 template <typename ST>
 __device__ void naive_pass_fwd(int dir, const ST* xp, const ST* wp, const ST* lp, const ST* up,
-                               const ST* h0p, float* hbuf, float* hall, float* ysm, int H, int W) {
+                               const ST* h0p, float* hbuf, float* hall, float* ysm, int H, int W, int Lc) {
     const int Ls = dir < 2 ? H : W, Lp = dir < 2 ? W : H;
     const int Lmax = H > W ? H : W;
     const int plane = H * W;
@@ -51,9 +58,11 @@ __device__ void naive_pass_fwd(int dir, const ST* xp, const ST* wp, const ST* lp
                 if (p < Lp) {
                     const int o = img_off(dir, s, p, H, W);
                     float acc = lx[j];
-                    if (p > 0)      acc = fmaf(w0[j], cur[p], acc);
-                    acc = fmaf(w1[j], cur[p + 1], acc);
-                    if (p < Lp - 1) acc = fmaf(w2[j], cur[p + 2], acc);
+                    if (!band_entry(dir, s, Ls, Lc)) {
+                        if (p > 0)      acc = fmaf(w0[j], cur[p], acc);
+                        acc = fmaf(w1[j], cur[p + 1], acc);
+                        if (p < Lp - 1) acc = fmaf(w2[j], cur[p + 2], acc);
+                    }
                     nxt[p + 1] = acc;
                     if (hall) hall[o] = acc;
                     if (ysm) ysm[o] = fmaf(uu[j], acc, ysm[o]);
@@ -94,7 +103,7 @@ __global__ void naive_fwd_kernel(FwdArgs<ST> a) {
         const SlabIn in(sh, q, b, c, g);
         naive_pass_fwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + in.w * 3 * plane,
                            a.lam + in.l * plane, a.u + in.u * plane,
-                           a.h0 ? a.h0 + dbc * Lmax : nullptr, hbuf, nullptr, ysm, H, W);
+                           a.h0 ? a.h0 + dbc * Lmax : nullptr, hbuf, nullptr, ysm, H, W, sh.band(dir < 2 ? H : W));
         ++q;
     }
     __syncthreads();
@@ -109,7 +118,7 @@ __global__ void naive_fwd_kernel(FwdArgs<ST> a) {
 template <typename ST>
 __device__ void naive_pass_bwd(int dir, const ST* xp, const ST* wp, const ST* lp, const ST* up,
                                const ST* h0p, const ST* gyp, const float* hall, float* ghs,
-                               float* dxs, float* dws, ST* dlp, ST* dup, ST* dh0p, int H, int W) {
+                               float* dxs, float* dws, ST* dlp, ST* dup, ST* dh0p, int H, int W, int Lc) {
     const int Ls = dir < 2 ? H : W, Lp = dir < 2 ? W : H;
     const int Lmax = H > W ? H : W;
     const int plane = H * W;
@@ -145,7 +154,7 @@ __device__ void naive_pass_bwd(int dir, const ST* xp, const ST* wp, const ST* lp
                     if (dup) st_f(dup + o, gy * hall[o]);
                     if (dxs) dxs[o] = fmaf(lv[j], gh, dxs[o]);
                     if (dlp) st_f(dlp + o, xv[j] * gh);
-                    if (dws) {
+                    if (dws && !band_entry(dir, s, Ls, Lc)) {      // a band's first step multiplies a zero state: no dw3 term
 #pragma unroll
                         for (int k = 0; k < 3; ++k) {
                             const int pn = p + k - 1;
@@ -164,7 +173,7 @@ __device__ void naive_pass_bwd(int dir, const ST* xp, const ST* wp, const ST* lp
                     if (p > 0)      acc = fmaf(wl[j], ghs[p], acc);
                     acc = fmaf(wc[j], ghs[p + 1], acc);
                     if (p < Lp - 1) acc = fmaf(wr[j], ghs[p + 2], acc);
-                    carry = acc;
+                    carry = band_entry(dir, s, Ls, Lc) ? 0.f : acc;      // nothing flows back across a band's first step
                 }
                 __syncthreads();
             }
@@ -195,14 +204,15 @@ __global__ void naive_bwd_main_kernel(BwdArgs<ST> a) {
         const size_t dbc = ((size_t)q * sh.B + b) * sh.C + c;
         const SlabIn in(sh, q, b, c, g);
         const ST* h0p = a.h0 ? a.h0 + dbc * Lmax : nullptr;
+        const int Lc = sh.band(dir < 2 ? H : W);
         naive_pass_fwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + in.w * 3 * plane,
-                           a.lam + in.l * plane, a.u + in.u * plane, h0p, hbuf, hall, nullptr, H, W);
+                           a.lam + in.l * plane, a.u + in.u * plane, h0p, hbuf, hall, nullptr, H, W, Lc);
         naive_pass_bwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + in.w * 3 * plane,
                            a.lam + in.l * plane, a.u + in.u * plane, h0p, a.dy + (size_t)bc * plane,
                            hall, ghs, a.dx ? dxs : nullptr, nullptr,
                            a.dlam ? a.dlam + dbc * plane : nullptr,
                            a.du ? a.du + dbc * plane : nullptr,
-                           a.dh0 ? a.dh0 + dbc * Lmax : nullptr, H, W);
+                           a.dh0 ? a.dh0 + dbc * Lmax : nullptr, H, W, Lc);
         __syncthreads();
         ++q;
     }
@@ -230,6 +240,7 @@ __global__ void naive_bwd_dw_kernel(BwdArgs<ST> a) {
     for (int o = threadIdx.x; o < 3 * plane; o += blockDim.x) dws[o] = 0.f;
     __syncthreads();
     const size_t dbg = ((size_t)q * sh.B + b) * sh.G + g;
+    const int Lc = sh.band(dir < 2 ? H : W);
     for (int cc = 0; cc < cg; ++cc) {
         const int c = g * cg + cc;
         const size_t bc = (size_t)b * sh.C + c;
@@ -237,10 +248,10 @@ __global__ void naive_bwd_dw_kernel(BwdArgs<ST> a) {
         const SlabIn in(sh, q, b, c, g);
         const ST* h0p = a.h0 ? a.h0 + dbc * Lmax : nullptr;
         naive_pass_fwd<ST>(dir, a.x + bc * plane, a.w3 + in.w * 3 * plane, a.lam + in.l * plane,
-                           a.u + in.u * plane, h0p, hbuf, hall, nullptr, H, W);
+                           a.u + in.u * plane, h0p, hbuf, hall, nullptr, H, W, Lc);
         naive_pass_bwd<ST>(dir, a.x + bc * plane, a.w3 + in.w * 3 * plane, a.lam + in.l * plane,
                            a.u + in.u * plane, h0p, a.dy + bc * plane, hall, ghs, nullptr, dws,
-                           nullptr, nullptr, nullptr, H, W);
+                           nullptr, nullptr, nullptr, H, W, Lc);
         __syncthreads();
     }
     ST* dwp = a.dw3 + dbg * 3 * plane;

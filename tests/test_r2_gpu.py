@@ -340,3 +340,37 @@ def test_shared_direction_slabs(dtype, shared):
     with pytest.raises(gspn.GspnError) as ei:
         gspn.gspn_scan_fwd(d["x"], one["w3"], one["lam"], one["u"], cfg.G, mask, shared=shared, impl=gspn.IMPL_CHAIN)
     assert ei.value.status == 2
+
+
+# ---------------------------------------------------------------------------------- chunked scan
+@pytest.mark.parametrize("k_chunk", [2, 3, 7])
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_chunked_scan_matches_the_oracle(dtype, k_chunk):
+    """gspn_args_t.k_chunk (reading 10): bands of ceil(L / k_chunk) lines in image coordinates, independent
+    scans with a zero initial state; forward and every gradient against oracle.fwd_chunked / bwd_chunked, with h0, ragged
+    last bands (37 / 3, 41 / 7, 70 / 3) and direction subsets; k_chunk = 1 is bit-identical to the plain call."""
+    from oracle import gspn_oracle as orc
+    for shape, mask in [((2, 4, 16, 16, 2), 15), ((1, 4, 37, 41, 2), 15), ((2, 2, 27, 27, 1), 6), ((1, 2, 70, 33, 1), 9)]:
+        cfg = gi.small_config("chk", *shape, dir_mask=mask, seed=99, backward=True)
+        t = gi.make_inputs(cfg, dtype, device="cpu", with_dy=True, with_h0=True)
+        d = {k: v.cuda() for k, v in t.items()}
+        n = {k: pu.np64(v) for k, v in t.items()}
+        y = gspn.gspn_scan_fwd(d["x"], d["w3"], d["lam"], d["u"], cfg.G, mask, h0=d["h0"], k_chunk=k_chunk)
+        assert gspn.gspn_last_variant() == "naive_fwd"
+        yo = orc.fwd_chunked(n["x"], n["w3"], n["lam"], n["u"], cfg.G, mask, k_chunk, h0=n["h0"])
+        A = orc.fwd_chunked_magnitude(n["x"], n["w3"], n["lam"], n["u"], cfg.G, mask, k_chunk, h0=n["h0"])
+        r = pu.gate(pu.np64(y), yo, A, dtype)
+        assert r["ok"], (shape, mask, r)
+        g = gspn.gspn_scan_bwd(d["x"], d["w3"], d["lam"], d["u"], d["dy"], cfg.G, mask, h0=d["h0"], k_chunk=k_chunk)
+        assert gspn.gspn_last_variant() == "naive_bwd"
+        go = orc.bwd_chunked(n["x"], n["w3"], n["lam"], n["u"], n["dy"], cfg.G, mask, k_chunk, h0=n["h0"])
+        Ag = orc.bwd_chunked_magnitude(n["x"], n["w3"], n["lam"], n["u"], n["dy"], cfg.G, mask, k_chunk, h0=n["h0"])
+        for k in ("dx", "dlambda", "du", "dw3", "dh0"):
+            r = pu.gate(pu.np64(g[k]), go[k], Ag[k], dtype)
+            assert r["ok"], (shape, mask, k, r)
+        y1 = gspn.gspn_scan_fwd(d["x"], d["w3"], d["lam"], d["u"], cfg.G, mask, h0=d["h0"], k_chunk=1, impl=gspn.IMPL_NAIVE)
+        assert torch.equal(y1, gspn.gspn_scan_fwd(d["x"], d["w3"], d["lam"], d["u"], cfg.G, mask, h0=d["h0"], impl=gspn.IMPL_NAIVE))
+        assert not torch.equal(y1, y)                     # the bands matter
+    with pytest.raises(gspn.GspnError) as ei:
+        gspn.gspn_scan_fwd(d["x"], d["w3"], d["lam"], d["u"], cfg.G, mask, k_chunk=2, impl=gspn.IMPL_CHAIN)
+    assert ei.value.status == 2
