@@ -18,7 +18,7 @@ LIB = os.path.join(_HERE, "libgspn.so")
 
 SOURCES = ["gspn_api.cu", "gspn_naive.cu", "gspn_merge.cu", "gspn_tmap.cu", "gspn_fused_fwd.cu", "gspn_group_bwd.cu",
            "gspn_flat_fwd.cu", "gspn_chain_bwd.cu", "gspn_chain_fwd.cu", "gspn_pair_fwd.cu", "gspn_norm.cu", "gspn_plane_bwd.cu", "gspn_line_fwd.cu", "gspn_line_bwd.cu"]
-HEADERS = ["gspn_common.cuh", "gspn_kernels.h", "gspn_fused.cuh", "gspn_flat.cuh", "gspn_chain.cuh", "gspn_line.cuh"]
+HEADERS = ["gspn_common.cuh", "gspn_kernels.h", "gspn_fused.cuh", "gspn_flat.cuh", "gspn_chain.cuh", "gspn_line.cuh", "gspn_naive.cuh"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -1,0 +1,79 @@
+// naive_emu.cpp -- TEST ONLY.  Runs the DEVICE code of the naive kernels (paper_2606_00746_b200/csrc/gspn_naive.cuh, the
+// file the library compiles with nvcc) on the host: compiled with g++ against tests/emu/shim (a few lines standing in for
+// the CUDA headers), one thread block at a time, its threads as host threads, __syncthreads as a std::barrier.  It exists
+// so that a change to those kernels can be checked against the oracle on a machine without a GPU
+// (tests/test_naive_emulated_cpu.py).  It is not a CPU path of the library: nothing under paper_2606_00746_b200/ knows
+// about it, and it emulates nothing but the naive kernels' plain threadIdx / __syncthreads / shared-memory model.
+#include <thread>
+#include <vector>
+
+#include "gspn_naive.cuh"
+
+namespace emu {
+thread_local uint3 tid;
+uint3 bid;
+dim3 bdim, gdim;
+std::barrier<>* block_barrier;
+}  // namespace emu
+
+namespace gspn {
+float smem[1 << 20];      // dynamic shared memory of the running block (4 MB: far above the 227 KB a real CTA has)
+}
+
+template <typename F>
+static void run_grid(unsigned blocks, unsigned threads, F kernel) {
+    emu::gdim.x = blocks;
+    emu::bdim.x = threads;
+    for (unsigned b = 0; b < blocks; ++b) {
+        emu::bid = uint3{b, 0, 0};
+        std::barrier<> bar((std::ptrdiff_t)threads);
+        emu::block_barrier = &bar;
+        std::vector<std::thread> pool;
+        for (unsigned t = 0; t < threads; ++t)
+            pool.emplace_back([=] { emu::tid = uint3{t, 0, 0}; kernel(); });
+        for (auto& th : pool) th.join();
+    }
+}
+
+static int round_up32(int v) { return (v + 31) / 32 * 32; }
+
+template <typename ST>
+static int fwd_t(const void* x, const void* w3, const void* lam, const void* u, const void* h0, void* y, gspn::Shape sh) {
+    gspn::FwdArgs<ST> a{(const ST*)x, (const ST*)w3, (const ST*)lam, (const ST*)u, (const ST*)h0, (ST*)y, sh};
+    if ((sh.plane() + 2 * (sh.Lmax() + 2)) > sizeof(gspn::smem) / 4) return 2;
+    run_grid(sh.B * sh.C, round_up32(sh.Lmax()), [=] { gspn::naive_fwd_kernel<ST>(a); });      // grid / block of naive_fwd_launch
+    return 0;
+}
+
+template <typename ST>
+static int bwd_t(const void* x, const void* w3, const void* lam, const void* u, const void* h0, const void* dy, void* dx,
+                 void* dlam, void* du, void* dw3, void* dh0, gspn::Shape sh) {
+    gspn::BwdArgs<ST> a{(const ST*)x, (const ST*)w3, (const ST*)lam, (const ST*)u, (const ST*)h0, (const ST*)dy,
+                        (ST*)dx, (ST*)dlam, (ST*)du, (ST*)dw3, (ST*)dh0, sh};
+    if ((4 * sh.plane() + 3 * (sh.Lmax() + 2)) > sizeof(gspn::smem) / 4) return 2;
+    // the two launches of naive_bwd_launch, same grids and blocks
+    if (a.dx || a.dlam || a.du || a.dh0)
+        run_grid(sh.B * sh.C, round_up32(sh.Lmax()), [=] { gspn::naive_bwd_main_kernel<ST>(a); });
+    if (a.dw3)
+        run_grid(sh.D() * sh.B * sh.G, round_up32(sh.Lmax()), [=] { gspn::naive_bwd_dw_kernel<ST>(a); });
+    return 0;
+}
+
+extern "C" {
+
+// dtype: 0 fp32, 1 bf16 (include/gspn.h); shared: bits of gspn::kShared*; k_chunk as gspn_args_t.k_chunk
+int emu_naive_fwd(const void* x, const void* w3, const void* lam, const void* u, const void* h0, void* y, int B, int C, int H,
+                  int W, int G, unsigned mask, unsigned shared, int k_chunk, int dtype) {
+    const gspn::Shape sh{B, C, H, W, G, mask, shared, k_chunk};
+    return dtype == 0 ? fwd_t<float>(x, w3, lam, u, h0, y, sh) : fwd_t<__nv_bfloat16>(x, w3, lam, u, h0, y, sh);
+}
+
+int emu_naive_bwd(const void* x, const void* w3, const void* lam, const void* u, const void* h0, const void* dy, void* dx,
+                  void* dlam, void* du, void* dw3, void* dh0, int B, int C, int H, int W, int G, unsigned mask,
+                  unsigned shared, int k_chunk, int dtype) {
+    const gspn::Shape sh{B, C, H, W, G, mask, shared, k_chunk};
+    return dtype == 0 ? bwd_t<float>(x, w3, lam, u, h0, dy, dx, dlam, du, dw3, dh0, sh)
+                      : bwd_t<__nv_bfloat16>(x, w3, lam, u, h0, dy, dx, dlam, du, dw3, dh0, sh);
+}
+
+}  // extern "C"

@@ -1,0 +1,13 @@
+// Shim of <cuda_bf16.h> for tests/emu (TEST ONLY): storage type and round-to-nearest-even conversion.
+#pragma once
+#include <cstdint>
+#include <cstring>
+struct __nv_bfloat16 { unsigned short x; };
+inline __nv_bfloat16 __float2bfloat16_rn(float f) {
+    uint32_t v; std::memcpy(&v, &f, 4);
+    __nv_bfloat16 r;
+    if ((v & 0x7fffffffu) > 0x7f800000u) { r.x = 0x7fff; return r; }      // NaN
+    v += 0x7fffu + ((v >> 16) & 1u);                                      // round to nearest, ties to even
+    r.x = (unsigned short)(v >> 16);
+    return r;
+}

@@ -1,0 +1,165 @@
+"""The DEVICE code of the naive kernels (csrc/gspn_naive.cuh), run on the host by tests/emu/naive_emu.cpp, against the
+oracle -- on a machine without a GPU.
+
+Why: GPU access for this repository closed in round 2 before the shared-slab (`dir_stride_* = 0`) and chunked-scan
+(`k_chunk`) options of the naive kernels could run on hardware.  The naive kernels use nothing but threadIdx,
+__syncthreads and shared memory, so the very file nvcc compiles can be compiled by g++ against a small shim and run one
+thread block at a time with host threads.  What this checks is the kernels' index arithmetic and control flow (the same
+source); what it cannot check is anything specific to the GPU (launch configuration limits, fma contraction by nvcc is
+not at play: the kernels call fmaf explicitly, which the host evaluates with the same single rounding).
+The GPU parity tests (tests/test_parity_gpu.py, tests/test_r2_gpu.py) remain the parity evidence; this is the
+CPU-side safety net under them.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+import pytest
+import torch
+
+import gspn_inputs as gi
+import parity_util as pu
+from oracle import gspn_oracle as orc
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+EMU = os.path.join(HERE, "emu")
+CSRC = os.path.join(os.path.dirname(HERE), "paper_2606_00746_b200", "csrc")
+LIB = os.path.join(EMU, "libnaive_emu.so")
+SHARED_BITS = {"w3": 1, "lam": 2, "u": 4}
+
+
+@pytest.fixture(scope="module")
+def emu():
+    srcs = [os.path.join(EMU, "naive_emu.cpp"), os.path.join(EMU, "shim", "cuda_runtime.h"), os.path.join(EMU, "shim", "cuda_bf16.h"),
+            os.path.join(CSRC, "gspn_naive.cuh"), os.path.join(CSRC, "gspn_common.cuh")]
+    if not os.path.exists(LIB) or os.path.getmtime(LIB) < max(os.path.getmtime(s) for s in srcs):
+        cmd = ["g++", "-std=c++20", "-O1", "-pthread", "-fPIC", "-shared", "-ffp-contract=off", "-I", os.path.join(EMU, "shim"),
+               "-I", CSRC, "-o", LIB + ".tmp", srcs[0]]
+        subprocess.run(cmd, check=True)
+        os.replace(LIB + ".tmp", LIB)
+    L = ctypes.CDLL(LIB)
+    vp, ci, cu = ctypes.c_void_p, ctypes.c_int, ctypes.c_uint
+    L.emu_naive_fwd.argtypes = [vp] * 6 + [ci] * 5 + [cu, cu, ci, ci]
+    L.emu_naive_bwd.argtypes = [vp] * 11 + [ci] * 5 + [cu, cu, ci, ci]
+    return L
+
+
+def to_dev(t: torch.Tensor) -> np.ndarray:
+    """Storage bytes of a tensor as the kernels see them (bf16 as uint16)."""
+    t = t.contiguous()
+    return t.view(torch.int16).numpy().view(np.uint16).copy() if t.dtype == torch.bfloat16 else t.numpy().copy()
+
+
+def from_dev(a: np.ndarray, dtype: str) -> np.ndarray:
+    if dtype == "bf16":
+        return (a.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+    return a.astype(np.float64)
+
+
+def ptr(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def run_fwd(L, cfg, dtype, t, shared=(), k_chunk=0):
+    d = {k: to_dev(v[0] if k in shared else v) for k, v in t.items()}
+    y = np.full_like(d["x"], 0x7fc1 if dtype == "bf16" else np.nan)
+    rc = L.emu_naive_fwd(ptr(d["x"]), ptr(d["w3"]), ptr(d["lam"]), ptr(d["u"]), ptr(d.get("h0")), ptr(y), cfg.B, cfg.C, cfg.H,
+                         cfg.W, cfg.G, cfg.dir_mask, sum(SHARED_BITS[k] for k in shared), k_chunk, 0 if dtype == "f32" else 1)
+    assert rc == 0
+    return from_dev(y, dtype)
+
+
+def run_bwd(L, cfg, dtype, t, shared=(), k_chunk=0, need=("dx", "dlambda", "du", "dw3", "dh0")):
+    d = {k: to_dev(v[0] if k in shared else v) for k, v in t.items()}
+    full = {k: to_dev(v) for k, v in t.items()}
+    st = full["x"].dtype
+    fill = 0x7fc1 if dtype == "bf16" else np.nan
+    shapes = {"dx": full["x"].shape, "dlambda": full["lam"].shape, "du": full["u"].shape, "dw3": full["w3"].shape,
+              "dh0": (cfg.D, cfg.B, cfg.C, max(cfg.H, cfg.W))}
+    out = {k: np.full(shapes[k], fill, dtype=st) for k in need}
+    g = lambda k: ptr(out.get(k))
+    rc = L.emu_naive_bwd(ptr(d["x"]), ptr(d["w3"]), ptr(d["lam"]), ptr(d["u"]), ptr(d.get("h0")), ptr(d["dy"]), g("dx"), g("dlambda"),
+                         g("du"), g("dw3"), g("dh0"), cfg.B, cfg.C, cfg.H, cfg.W, cfg.G, cfg.dir_mask,
+                         sum(SHARED_BITS[k] for k in shared), k_chunk, 0 if dtype == "f32" else 1)
+    assert rc == 0
+    return {k: from_dev(v, dtype) for k, v in out.items()}
+
+
+CASES = [((2, 4, 8, 8, 2), 15), ((1, 4, 13, 17, 2), 15), ((1, 2, 33, 9, 1), 6), ((2, 2, 5, 40, 2), 9), ((1, 1, 1, 6, 1), 15),
+         ((1, 2, 7, 1, 1), 15)]
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("shape,mask", CASES, ids=["x".join(map(str, s)) + f"-m{m}" for s, m in CASES])
+def test_naive_kernels_emulated_match_the_oracle(emu, shape, mask, dtype):
+    """The plain operator (what round 1 measured on hardware): forward and every gradient, with h0."""
+    cfg = gi.small_config("emu", *shape, dir_mask=mask, seed=123, backward=True)
+    t = gi.make_inputs(cfg, dtype, device="cpu", with_dy=True, with_h0=True)
+    yo, A = pu.oracle_fwd(t, cfg)
+    r = pu.gate(run_fwd(emu, cfg, dtype, t), yo, A, dtype)
+    assert r["ok"], r
+    go, Ag = pu.oracle_bwd(t, cfg)
+    g = run_bwd(emu, cfg, dtype, t)
+    for k in go:
+        r = pu.gate(g[k], go[k], Ag[k], dtype)
+        assert r["ok"], (k, r)
+
+
+SHARED_SETS = [("w3",), ("lam", "u"), ("w3", "lam", "u")]
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("shared", SHARED_SETS, ids=["+".join(s) for s in SHARED_SETS])
+def test_shared_direction_slabs_emulated(emu, shared, dtype):
+    """dir_stride_* = 0: one slab read by every direction == the dense operator on the slab replicated D times."""
+    for shape, mask in [((2, 4, 9, 11, 2), 15), ((1, 2, 12, 7, 1), 6), ((1, 2, 6, 14, 2), 9)]:
+        cfg = gi.small_config("emus", *shape, dir_mask=mask, seed=124, backward=True)
+        t = gi.make_inputs(cfg, dtype, device="cpu", with_dy=True, with_h0=True)
+        rep = dict(t)
+        for k in shared:
+            rep[k] = t[k][:1].expand(cfg.D, *t[k].shape[1:]).contiguous()
+        yo, A = pu.oracle_fwd(rep, cfg)
+        y = run_fwd(emu, cfg, dtype, t, shared=shared)
+        r = pu.gate(y, yo, A, dtype)
+        assert r["ok"], (shape, mask, r)
+        np.testing.assert_array_equal(y, run_fwd(emu, cfg, dtype, rep))          # same kernel, same arithmetic
+        go, Ag = pu.oracle_bwd(rep, cfg)
+        g = run_bwd(emu, cfg, dtype, t, shared=shared)
+        gd = run_bwd(emu, cfg, dtype, rep)
+        for k in go:
+            r = pu.gate(g[k], go[k], Ag[k], dtype)
+            assert r["ok"], (shape, mask, k, r)
+            np.testing.assert_array_equal(g[k], gd[k], err_msg=k)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("k_chunk", [2, 3, 7])
+def test_chunked_scan_emulated(emu, k_chunk, dtype):
+    """k_chunk > 1 against oracle fwd_chunked / bwd_chunked, with h0, ragged bands and direction subsets."""
+    for shape, mask in [((2, 4, 8, 8, 2), 15), ((1, 2, 13, 17, 1), 15), ((1, 2, 10, 9, 2), 6), ((1, 2, 11, 20, 1), 9)]:
+        cfg = gi.small_config("emuc", *shape, dir_mask=mask, seed=125, backward=True)
+        t = gi.make_inputs(cfg, dtype, device="cpu", with_dy=True, with_h0=True)
+        n = {k: pu.np64(v) for k, v in t.items()}
+        yo = orc.fwd_chunked(n["x"], n["w3"], n["lam"], n["u"], cfg.G, mask, k_chunk, h0=n["h0"])
+        A = orc.fwd_chunked_magnitude(n["x"], n["w3"], n["lam"], n["u"], cfg.G, mask, k_chunk, h0=n["h0"])
+        y = run_fwd(emu, cfg, dtype, t, k_chunk=k_chunk)
+        r = pu.gate(y, yo, A, dtype)
+        assert r["ok"], (shape, mask, r)
+        go = orc.bwd_chunked(n["x"], n["w3"], n["lam"], n["u"], n["dy"], cfg.G, mask, k_chunk, h0=n["h0"])
+        Ag = orc.bwd_chunked_magnitude(n["x"], n["w3"], n["lam"], n["u"], n["dy"], cfg.G, mask, k_chunk, h0=n["h0"])
+        g = run_bwd(emu, cfg, dtype, t, k_chunk=k_chunk)
+        for k in go:
+            r = pu.gate(g[k], go[k], Ag[k], dtype)
+            assert r["ok"], (shape, mask, k, r)
+        np.testing.assert_array_equal(run_fwd(emu, cfg, dtype, t, k_chunk=1), run_fwd(emu, cfg, dtype, t))
+
+
+def test_optional_outputs_emulated(emu):
+    cfg = gi.small_config("emuo", 1, 4, 9, 10, 2, seed=126, backward=True)
+    t = gi.make_inputs(cfg, "f32", device="cpu", with_dy=True)
+    full = run_bwd(emu, cfg, "f32", t)
+    for need in (("dx",), ("dw3",), ("du", "dh0"), ("dlambda", "dw3")):
+        part = run_bwd(emu, cfg, "f32", t, need=need)
+        for k in need:
+            np.testing.assert_array_equal(part[k], full[k])
