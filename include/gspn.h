@@ -159,7 +159,17 @@ typedef struct gspn_args {
      * belong to the band that holds the direction's scan step 0.  0 or 1 = the global scan; negative: GSPN_EINVAL.
      * k_chunk > 1 is served by the naive kernels only in this version (as shared slabs above). */
     int k_chunk;
+    /* r2 (second half; the paper's fused kernel consumes the logits).
+     * GSPN_FLAG_W3_LOGITS: `w3` holds the raw tap LOGITS [D,B,G,3,H,W] (or one shared slab) and Eq. 3 (gspn_normalize_fwd
+     * below: sigmoid, sum over the in-grid taps, clamp at GSPN_NORM_EPS, divide, out-of-grid taps 0) is applied where the
+     * scan loads its taps, in fp32: the normalised taps are never written to memory and never rounded to the storage
+     * type.  The backward then writes to `dw3` the gradient of the LOGITS (Eq. 3's adjoint, gspn_normalize_bwd, applied on
+     * chip to the fp32 group sum; one rounding).  Other bits: GSPN_EINVAL.  Served by the naive kernels only in this
+     * version (as shared slabs above). */
+    unsigned flags;
 } gspn_args_t;
+
+#define GSPN_FLAG_W3_LOGITS 1u
 
 #define GSPN_DIR_STRIDE_DENSE ((size_t)-1)
 #define GSPN_ARGS_SIZE_R1 (offsetof(gspn_args_t, dir_stride_w3))

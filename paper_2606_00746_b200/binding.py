@@ -45,7 +45,10 @@ class _Args(ctypes.Structure):
                 ("G", ctypes.c_int), ("dir_mask", ctypes.c_uint), ("dtype", ctypes.c_int),
                 ("impl", ctypes.c_int), ("stream", ctypes.c_void_p),
                 ("dir_stride_w3", ctypes.c_size_t), ("dir_stride_lambda", ctypes.c_size_t),
-                ("dir_stride_u", ctypes.c_size_t), ("k_chunk", ctypes.c_int)]
+                ("dir_stride_u", ctypes.c_size_t), ("k_chunk", ctypes.c_int), ("flags", ctypes.c_uint)]
+
+
+FLAG_W3_LOGITS = 1
 
 
 DIR_STRIDE_DENSE = ctypes.c_size_t(-1).value       # GSPN_DIR_STRIDE_DENSE
@@ -135,9 +138,10 @@ def _shapes(x, G, dir_mask):
 
 
 def gspn_scan_fwd(x, w3, lam, u, G: int, dir_mask: int = DIR_ALL, h0=None, out=None,
-                  impl: int = IMPL_AUTO, shared=(), k_chunk: int = 0):
+                  impl: int = IMPL_AUTO, shared=(), k_chunk: int = 0, w3_logits: bool = False):
     """y = sum_d u_d * scan_d(x); see include/gspn.h gspn_scan_fwd / gspn_scan_fwd_ex.
     k_chunk > 1: the chunked scan (bands of ceil(L / k_chunk) lines, independent scans; gspn_args_t.k_chunk).
+    w3_logits: w3 holds the raw tap logits, Eq. 3 is applied where the taps are loaded (GSPN_FLAG_W3_LOGITS).
     shared: operands among ("w3", "lam", "u") that hold ONE slab ([B,G,3,H,W] / [B,C,H,W], no D axis) read by every
     direction (gspn_args_t.dir_stride_* = 0)."""
     if not x.is_cuda:
@@ -148,7 +152,7 @@ def gspn_scan_fwd(x, w3, lam, u, G: int, dir_mask: int = DIR_ALL, h0=None, out=N
     _dev(h0, "h0", s_h0, x)
     y = torch.empty_like(x) if out is None else _dev(out, "out", x.shape, x)
     with torch.cuda.device(x.device):
-        if h0 is None and impl == IMPL_AUTO and not shared and k_chunk <= 1:
+        if h0 is None and impl == IMPL_AUTO and not shared and k_chunk <= 1 and not w3_logits:
             rc = lib().gspn_scan_fwd(_p(x), _p(w3), _p(lam), _p(u), _p(y), B, C, H, W, G, dir_mask,
                                      _dtype_code(x), _stream(x))
         else:
@@ -156,16 +160,18 @@ def gspn_scan_fwd(x, w3, lam, u, G: int, dir_mask: int = DIR_ALL, h0=None, out=N
                       lam=lam.data_ptr(), u=u.data_ptr(), h0=None if h0 is None else h0.data_ptr(),
                       y=y.data_ptr(), B=B, C=C, H=H, W=W, G=G, dir_mask=dir_mask,
                       dtype=_dtype_code(x), impl=impl,
-                      stream=torch.cuda.current_stream(x.device).cuda_stream, k_chunk=k_chunk, **_strides(shared))
+                      stream=torch.cuda.current_stream(x.device).cuda_stream, k_chunk=k_chunk, flags=FLAG_W3_LOGITS if w3_logits else 0, **_strides(shared))
             rc = lib().gspn_scan_fwd_ex(ctypes.byref(a))
     _check(rc)
     return y
 
 
 def gspn_scan_bwd(x, w3, lam, u, dy, G: int, dir_mask: int = DIR_ALL, h0=None,
-                  need=("dx", "dlambda", "du", "dw3", "dh0"), impl: int = IMPL_AUTO, shared=(), k_chunk: int = 0) -> dict:
+                  need=("dx", "dlambda", "du", "dw3", "dh0"), impl: int = IMPL_AUTO, shared=(), k_chunk: int = 0,
+                  w3_logits: bool = False) -> dict:
     """Adjoint of gspn_scan_fwd; returns the requested gradients (include/gspn.h gspn_scan_bwd).
-    shared: as in gspn_scan_fwd; the gradients keep one slab per direction (the gradient of a shared slab is their sum)."""
+    shared: as in gspn_scan_fwd; the gradients keep one slab per direction (the gradient of a shared slab is their sum).
+    w3_logits: w3 holds logits; "dw3" is then the gradient of the logits."""
     if not x.is_cuda:
         raise ValueError("x: need a CUDA tensor (there is no CPU path)")
     B, C, H, W, D, s_bc, s_w, s_h0 = _shapes(x, G, dir_mask)
@@ -176,7 +182,7 @@ def gspn_scan_bwd(x, w3, lam, u, dy, G: int, dir_mask: int = DIR_ALL, h0=None,
     out = {k: torch.empty(shapes[k], dtype=x.dtype, device=x.device) for k in need}
     g = lambda k: out[k].data_ptr() if k in out else None
     with torch.cuda.device(x.device):
-        if h0 is None and impl == IMPL_AUTO and not shared and k_chunk <= 1:
+        if h0 is None and impl == IMPL_AUTO and not shared and k_chunk <= 1 and not w3_logits:
             rc = lib().gspn_scan_bwd(_p(x), _p(w3), _p(lam), _p(u), _p(dy), g("dx"), g("dlambda"),
                                      g("du"), g("dw3"), g("dh0"), B, C, H, W, G, dir_mask,
                                      _dtype_code(x), _stream(x))
@@ -186,7 +192,7 @@ def gspn_scan_bwd(x, w3, lam, u, dy, G: int, dir_mask: int = DIR_ALL, h0=None,
                       dy=dy.data_ptr(), dx=g("dx"), dlambda=g("dlambda"), du=g("du"), dw3=g("dw3"),
                       dh0=g("dh0"), B=B, C=C, H=H, W=W, G=G, dir_mask=dir_mask,
                       dtype=_dtype_code(x), impl=impl,
-                      stream=torch.cuda.current_stream(x.device).cuda_stream, k_chunk=k_chunk, **_strides(shared))
+                      stream=torch.cuda.current_stream(x.device).cuda_stream, k_chunk=k_chunk, flags=FLAG_W3_LOGITS if w3_logits else 0, **_strides(shared))
             rc = lib().gspn_scan_bwd_ex(ctypes.byref(a))
     _check(rc)
     return out

@@ -52,19 +52,20 @@ static unsigned shared_bits(const gspn_args_t* a) {
            (a->dir_stride_u == 0 ? kSharedU : 0u);
 }
 static int chunks(const gspn_args_t* a) { return a->struct_size == GSPN_ARGS_SIZE_R1 ? 0 : a->k_chunk; }
+static unsigned arg_flags(const gspn_args_t* a) { return a->struct_size == GSPN_ARGS_SIZE_R1 ? 0u : a->flags; }
 
 template <typename ST>
 static int fwd_typed(const gspn_args_t* a) {
     FwdArgs<ST> f;
     f.x = (const ST*)a->x; f.w3 = (const ST*)a->w3; f.lam = (const ST*)a->lambda;
     f.u = (const ST*)a->u; f.h0 = (const ST*)a->h0; f.y = (ST*)a->y;
-    f.sh = Shape{a->B, a->C, a->H, a->W, a->G, a->dir_mask, shared_bits(a), chunks(a)};
+    f.sh = Shape{a->B, a->C, a->H, a->W, a->G, a->dir_mask, shared_bits(a), chunks(a), arg_flags(a)};
     cudaStream_t st = (cudaStream_t)a->stream;
     LaunchInfo li{0, ""};
     int rc;
-    if (f.sh.shared || f.sh.k_chunk > 1) {      // shared slabs, chunked scan: the naive kernel only (include/gspn.h)
+    if (f.sh.shared || f.sh.k_chunk > 1 || f.sh.flags) {      // shared slabs, chunked scan, logits: the naive kernel only (include/gspn.h)
         if (a->impl != GSPN_IMPL_AUTO && a->impl != GSPN_IMPL_NAIVE) {
-            set_error("shared direction slabs (dir_stride_* = 0) and k_chunk > 1 are served by the naive kernels only (impl %d asked)", a->impl);
+            set_error("shared direction slabs (dir_stride_* = 0), k_chunk > 1 and GSPN_FLAG_W3_LOGITS are served by the naive kernels only (impl %d asked)", a->impl);
             return GSPN_EUNSUPPORTED;
         }
         rc = naive_fwd_launch<ST>(f, st, &li);
@@ -103,13 +104,13 @@ static int bwd_typed(const gspn_args_t* a) {
     f.u = (const ST*)a->u; f.h0 = (const ST*)a->h0; f.dy = (const ST*)a->dy;
     f.dx = (ST*)a->dx; f.dlam = (ST*)a->dlambda; f.du = (ST*)a->du; f.dw3 = (ST*)a->dw3;
     f.dh0 = (ST*)a->dh0;
-    f.sh = Shape{a->B, a->C, a->H, a->W, a->G, a->dir_mask, shared_bits(a), chunks(a)};
+    f.sh = Shape{a->B, a->C, a->H, a->W, a->G, a->dir_mask, shared_bits(a), chunks(a), arg_flags(a)};
     cudaStream_t st = (cudaStream_t)a->stream;
     LaunchInfo li{0, ""};
     int rc;
-    if (f.sh.shared || f.sh.k_chunk > 1) {
+    if (f.sh.shared || f.sh.k_chunk > 1 || f.sh.flags) {
         if (a->impl != GSPN_IMPL_AUTO && a->impl != GSPN_IMPL_NAIVE) {
-            set_error("shared direction slabs (dir_stride_* = 0) and k_chunk > 1 are served by the naive kernels only (impl %d asked)", a->impl);
+            set_error("shared direction slabs (dir_stride_* = 0), k_chunk > 1 and GSPN_FLAG_W3_LOGITS are served by the naive kernels only (impl %d asked)", a->impl);
             return GSPN_EUNSUPPORTED;
         }
         rc = naive_bwd_launch<ST>(f, st, &li);
@@ -164,6 +165,7 @@ static int check_ex(const gspn_args_t* a) {
                 return GSPN_EINVAL;
             }
         if (a->k_chunk < 0) { set_error("k_chunk=%d is negative (0 or 1 = the global scan)", a->k_chunk); return GSPN_EINVAL; }
+        if (a->flags & ~GSPN_FLAG_W3_LOGITS) { set_error("flags=0x%x: unknown bit(s)", a->flags); return GSPN_EINVAL; }
     }
     return GSPN_OK;
 }

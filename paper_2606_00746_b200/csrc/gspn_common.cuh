@@ -29,6 +29,7 @@ __device__ __forceinline__ int img_off(int dir, int s, int p, int H, int W) {
 }
 
 constexpr unsigned kSharedW3 = 1u, kSharedLam = 2u, kSharedU = 4u;
+constexpr unsigned kFlagLogits = 1u;
 
 struct Shape {
     int B, C, H, W, G;
@@ -39,6 +40,10 @@ struct Shape {
     // chunked scan (gspn_args_t.k_chunk, reading 10): bands of ceil(L / k_chunk) lines of the scan axis in image
     // coordinates, each an independent scan with a zero initial state.  0 or 1 = one band (the global scan).
     int k_chunk;
+    // kFlagLogits: `w3` holds the raw tap LOGITS and Eq. 3 is applied where the taps are loaded (gspn_args_t.flags,
+    // SURVEY 8(f) f1, second half); the backward then writes the gradient of the logits to dw3
+    unsigned flags;
+    __host__ __device__ bool logits() const { return (flags & 1u) != 0; }
     __host__ __device__ int band(int Ls) const { const int k = k_chunk > 1 ? k_chunk : 1; return (Ls + k - 1) / k; }
     __host__ __device__ int cg() const { return C / G; }
     __host__ __device__ int Lmax() const { return H > W ? H : W; }

@@ -7,6 +7,45 @@
 
 namespace gspn {
 
+// ---- Eq. 3 in the load path (Shape::logits(); include/gspn.h gspn_normalize_fwd) --------------------
+// s_k = sigmoid(l_k), S = sum over the taps whose neighbour is inside the grid, w_k = s_k / max(S, eps), 0 outside.
+constexpr float kNormEps = 1e-6f;      // GSPN_NORM_EPS of include/gspn.h (reading R17)
+struct Nrm3 {
+    float s[3], oms[3], w[3], S;       // sigmoid, 1 - sigmoid (as e * s: no cancellation), normalised tap, in-grid sum
+    bool v[3];
+};
+__device__ __forceinline__ Nrm3 nrm3(float l0, float l1, float l2, bool v0, bool v2) {
+    Nrm3 r;
+    const float l[3] = {l0, l1, l2};
+    r.v[0] = v0; r.v[1] = true; r.v[2] = v2;
+    r.S = 0.f;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const float e = expf(fminf(-l[k], 80.f));      // capped so that e stays finite: sigmoid(-80) = 1.8e-35 either way
+        r.s[k] = 1.f / (1.f + e);
+        r.oms[k] = e * r.s[k];
+        if (r.v[k]) r.S += r.s[k];
+    }
+    const float Sc = r.S > kNormEps ? r.S : kNormEps;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) r.w[k] = r.v[k] ? r.s[k] / Sc : 0.f;
+    return r;
+}
+
+// the three taps of the pixel at plane offset o, cross position p: the stored values (0 for a tap whose neighbour lies
+// outside the grid: it is never read), or Eq. 3 of the stored logits
+template <typename ST>
+__device__ __forceinline__ void load_taps(const ST* wp, int plane, int o, int p, int Lp, bool logits, float& w0, float& w1,
+                                          float& w2) {
+    w0 = p > 0 ? ld_f(wp + o) : 0.f;
+    w1 = ld_f(wp + plane + o);
+    w2 = p < Lp - 1 ? ld_f(wp + 2 * plane + o) : 0.f;
+    if (logits) {
+        const Nrm3 r = nrm3(w0, w1, w2, p > 0, p < Lp - 1);
+        w0 = r.w[0]; w1 = r.w[1]; w2 = r.w[2];
+    }
+}
+
 // one directional forward pass of one plane; every thread of the CTA must call it.
 //   hbuf : 2*(Lmax+2) floats, line s-1 / line s with a zero halo at both ends
 //   hall : NULL or [H*W] floats, receives every hidden state in image layout
@@ -22,7 +61,7 @@ __device__ __forceinline__ bool band_entry(int dir, int s, int Ls, int Lc) {
 
 template <typename ST>
 __device__ void naive_pass_fwd(int dir, const ST* xp, const ST* wp, const ST* lp, const ST* up,
-                               const ST* h0p, float* hbuf, float* hall, float* ysm, int H, int W, int Lc) {
+                               const ST* h0p, float* hbuf, float* hall, float* ysm, int H, int W, int Lc, bool logits) {
     const int Ls = dir < 2 ? H : W, Lp = dir < 2 ? W : H;
     const int Lmax = H > W ? H : W;
     const int plane = H * W;
@@ -42,9 +81,7 @@ __device__ void naive_pass_fwd(int dir, const ST* xp, const ST* wp, const ST* lp
             if (p < Lp && s0 + j < Ls) {
                 const int o = img_off(dir, s0 + j, p, H, W);
                 lx[j] = ld_f(lp + o) * ld_f(xp + o);
-                if (p > 0) w0[j] = ld_f(wp + o);
-                w1[j] = ld_f(wp + plane + o);
-                if (p < Lp - 1) w2[j] = ld_f(wp + 2 * plane + o);
+                load_taps<ST>(wp, plane, o, p, Lp, logits, w0[j], w1[j], w2[j]);
                 if (ysm) uu[j] = ld_f(up + o);
             }
         }
@@ -100,7 +137,7 @@ __global__ void naive_fwd_kernel(FwdArgs<ST> a) {
         const SlabIn in(sh, q, b, c, g);
         naive_pass_fwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + in.w * 3 * plane,
                            a.lam + in.l * plane, a.u + in.u * plane,
-                           a.h0 ? a.h0 + dbc * Lmax : nullptr, hbuf, nullptr, ysm, H, W, sh.band(dir < 2 ? H : W));
+                           a.h0 ? a.h0 + dbc * Lmax : nullptr, hbuf, nullptr, ysm, H, W, sh.band(dir < 2 ? H : W), sh.logits());
         ++q;
     }
     __syncthreads();
@@ -115,7 +152,7 @@ __global__ void naive_fwd_kernel(FwdArgs<ST> a) {
 template <typename ST>
 __device__ void naive_pass_bwd(int dir, const ST* xp, const ST* wp, const ST* lp, const ST* up,
                                const ST* h0p, const ST* gyp, const float* hall, float* ghs,
-                               float* dxs, float* dws, ST* dlp, ST* dup, ST* dh0p, int H, int W, int Lc) {
+                               float* dxs, float* dws, ST* dlp, ST* dup, ST* dh0p, int H, int W, int Lc, bool logits) {
     const int Ls = dir < 2 ? H : W, Lp = dir < 2 ? W : H;
     const int Lmax = H > W ? H : W;
     const int plane = H * W;
@@ -135,9 +172,16 @@ __device__ void naive_pass_bwd(int dir, const ST* xp, const ST* wp, const ST* lp
                 gyv[j] = ld_f(gyp + o); uv[j] = ld_f(up + o);
                 lv[j] = ld_f(lp + o);   xv[j] = ld_f(xp + o);
                 // taps of the carry w[s]^T gh: position p receives from p-1 (its tap k=2), p (k=1), p+1 (k=0)
-                if (p > 0)      wl[j] = ld_f(wp + 2 * plane + img_off(dir, s, p - 1, H, W));
-                wc[j] = ld_f(wp + plane + o);
-                if (p < Lp - 1) wr[j] = ld_f(wp + img_off(dir, s, p + 1, H, W));
+                if (!logits) {
+                    if (p > 0)      wl[j] = ld_f(wp + 2 * plane + img_off(dir, s, p - 1, H, W));
+                    wc[j] = ld_f(wp + plane + o);
+                    if (p < Lp - 1) wr[j] = ld_f(wp + img_off(dir, s, p + 1, H, W));
+                } else {            // each of the three taps belongs to another pixel: Eq. 3 of that pixel's logits
+                    float t0, t1, t2;
+                    if (p > 0) { load_taps<ST>(wp, plane, img_off(dir, s, p - 1, H, W), p - 1, Lp, true, t0, t1, t2); wl[j] = t2; }
+                    load_taps<ST>(wp, plane, o, p, Lp, true, t0, t1, t2); wc[j] = t1;
+                    if (p < Lp - 1) { load_taps<ST>(wp, plane, img_off(dir, s, p + 1, H, W), p + 1, Lp, true, t0, t1, t2); wr[j] = t0; }
+                }
             }
         }
 #pragma unroll
@@ -203,13 +247,13 @@ __global__ void naive_bwd_main_kernel(BwdArgs<ST> a) {
         const ST* h0p = a.h0 ? a.h0 + dbc * Lmax : nullptr;
         const int Lc = sh.band(dir < 2 ? H : W);
         naive_pass_fwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + in.w * 3 * plane,
-                           a.lam + in.l * plane, a.u + in.u * plane, h0p, hbuf, hall, nullptr, H, W, Lc);
+                           a.lam + in.l * plane, a.u + in.u * plane, h0p, hbuf, hall, nullptr, H, W, Lc, sh.logits());
         naive_pass_bwd<ST>(dir, a.x + (size_t)bc * plane, a.w3 + in.w * 3 * plane,
                            a.lam + in.l * plane, a.u + in.u * plane, h0p, a.dy + (size_t)bc * plane,
                            hall, ghs, a.dx ? dxs : nullptr, nullptr,
                            a.dlam ? a.dlam + dbc * plane : nullptr,
                            a.du ? a.du + dbc * plane : nullptr,
-                           a.dh0 ? a.dh0 + dbc * Lmax : nullptr, H, W, Lc);
+                           a.dh0 ? a.dh0 + dbc * Lmax : nullptr, H, W, Lc, sh.logits());
         __syncthreads();
         ++q;
     }
@@ -245,14 +289,41 @@ __global__ void naive_bwd_dw_kernel(BwdArgs<ST> a) {
         const SlabIn in(sh, q, b, c, g);
         const ST* h0p = a.h0 ? a.h0 + dbc * Lmax : nullptr;
         naive_pass_fwd<ST>(dir, a.x + bc * plane, a.w3 + in.w * 3 * plane, a.lam + in.l * plane,
-                           a.u + in.u * plane, h0p, hbuf, hall, nullptr, H, W, Lc);
+                           a.u + in.u * plane, h0p, hbuf, hall, nullptr, H, W, Lc, sh.logits());
         naive_pass_bwd<ST>(dir, a.x + bc * plane, a.w3 + in.w * 3 * plane, a.lam + in.l * plane,
                            a.u + in.u * plane, h0p, a.dy + bc * plane, hall, ghs, nullptr, dws,
-                           nullptr, nullptr, nullptr, H, W, Lc);
+                           nullptr, nullptr, nullptr, H, W, Lc, sh.logits());
         __syncthreads();
     }
     ST* dwp = a.dw3 + dbg * 3 * plane;
-    for (int o = threadIdx.x; o < 3 * plane; o += blockDim.x) st_f(dwp + o, dws[o]);
+    if (!sh.logits()) {
+        for (int o = threadIdx.x; o < 3 * plane; o += blockDim.x) st_f(dwp + o, dws[o]);
+        return;
+    }
+    // Eq. 3's adjoint on chip (include/gspn.h gspn_normalize_bwd): dws holds the gradient of the normalised taps; what is
+    // stored is the gradient of the logits:  dwt_k = s_k (1 - s_k) (dw_k - sum_{k' in N} dw_k' w_k') / S,  dw_k / eps
+    // in place of the bracket over S where the clamp is active, 0 for the out-of-grid taps.
+    const ST* wp = a.w3 + SlabIn(sh, q, b, g * cg, g).w * 3 * plane;
+    const int Lp = dir < 2 ? W : H;
+    for (int o = threadIdx.x; o < plane; o += blockDim.x) {
+        const int p = dir < 2 ? o % W : o / W;
+        const bool v0 = p > 0, v2 = p < Lp - 1;
+        const Nrm3 r = nrm3(v0 ? ld_f(wp + o) : 0.f, ld_f(wp + plane + o), v2 ? ld_f(wp + 2 * plane + o) : 0.f, v0, v2);
+        const float g3[3] = {dws[o], dws[plane + o], dws[2 * plane + o]};
+        const bool clamped = !(r.S > kNormEps);
+        float dot = 0.f;
+        if (!clamped) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k)
+                if (r.v[k]) dot = fmaf(g3[k], r.w[k], dot);
+        }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            float ds = 0.f;
+            if (r.v[k]) ds = clamped ? g3[k] / kNormEps : (g3[k] - dot) / r.S;
+            st_f(dwp + k * plane + o, r.s[k] * r.oms[k] * ds);
+        }
+    }
 }
 
 }  // namespace gspn

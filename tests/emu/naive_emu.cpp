@@ -61,17 +61,17 @@ static int bwd_t(const void* x, const void* w3, const void* lam, const void* u, 
 
 extern "C" {
 
-// dtype: 0 fp32, 1 bf16 (include/gspn.h); shared: bits of gspn::kShared*; k_chunk as gspn_args_t.k_chunk
+// dtype: 0 fp32, 1 bf16 (include/gspn.h); shared: bits of gspn::kShared*; k_chunk, flags as in gspn_args_t
 int emu_naive_fwd(const void* x, const void* w3, const void* lam, const void* u, const void* h0, void* y, int B, int C, int H,
-                  int W, int G, unsigned mask, unsigned shared, int k_chunk, int dtype) {
-    const gspn::Shape sh{B, C, H, W, G, mask, shared, k_chunk};
+                  int W, int G, unsigned mask, unsigned shared, int k_chunk, unsigned flags, int dtype) {
+    const gspn::Shape sh{B, C, H, W, G, mask, shared, k_chunk, flags};
     return dtype == 0 ? fwd_t<float>(x, w3, lam, u, h0, y, sh) : fwd_t<__nv_bfloat16>(x, w3, lam, u, h0, y, sh);
 }
 
 int emu_naive_bwd(const void* x, const void* w3, const void* lam, const void* u, const void* h0, const void* dy, void* dx,
                   void* dlam, void* du, void* dw3, void* dh0, int B, int C, int H, int W, int G, unsigned mask,
-                  unsigned shared, int k_chunk, int dtype) {
-    const gspn::Shape sh{B, C, H, W, G, mask, shared, k_chunk};
+                  unsigned shared, int k_chunk, unsigned flags, int dtype) {
+    const gspn::Shape sh{B, C, H, W, G, mask, shared, k_chunk, flags};
     return dtype == 0 ? bwd_t<float>(x, w3, lam, u, h0, dy, dx, dlam, du, dw3, dh0, sh)
                       : bwd_t<__nv_bfloat16>(x, w3, lam, u, h0, dy, dx, dlam, du, dw3, dh0, sh);
 }

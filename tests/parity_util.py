@@ -178,3 +178,24 @@ def check_norm(cfg: gi.ScanConfig, dtype: str, device: str = "cuda:0", batch_sli
         out["bwd"] = gate(np64(dwt), gref, norm_bwd_magnitude(wt64, dw64, cfg.dir_mask), dtype)
         out["ok"] = bool(out["ok"] and out["bwd"]["ok"])
     return out
+
+
+def oracle_logits(t: dict, wt: torch.Tensor, cfg: gi.ScanConfig, backward: bool = True):
+    """Oracle of the scan fed with tap LOGITS (GSPN_FLAG_W3_LOGITS, second half): the composition of two
+    pinned oracle functions, Eq. 3 (normalize) then the scan, and backwards the scan's adjoint then Eq. 3's adjoint.
+    Everything in fp64 from the storage-rounded logits; the normalised taps are never rounded (the kernel keeps them in
+    fp32 on chip).  Returns (y, A_y, grads, A_grads) with grads["dw3"] = the gradient of the logits."""
+    x, lam, u = (np64(t[k]) for k in ("x", "lam", "u"))
+    h0 = np64(t["h0"]) if "h0" in t else None
+    wl = np64(wt)
+    w3 = orc.normalize(wl, cfg.dir_mask)
+    y = orc.fwd(x, w3, lam, u, cfg.G, cfg.dir_mask, h0=h0)
+    A = orc.fwd_magnitude(x, w3, lam, u, cfg.G, cfg.dir_mask, h0=h0)
+    if not backward:
+        return y, A, None, None
+    dy = np64(t["dy"])
+    g = orc.bwd(x, w3, lam, u, dy, cfg.G, cfg.dir_mask, h0=h0)
+    Ag = orc.bwd_magnitude(x, w3, lam, u, dy, cfg.G, cfg.dir_mask, h0=h0)
+    g["dw3"], Ag["dw3"] = (orc.normalize_bwd(wl, g["dw3"], cfg.dir_mask),
+                           orc.normalize_bwd(wl, Ag["dw3"], cfg.dir_mask, magnitude=True))
+    return y, A, g, Ag

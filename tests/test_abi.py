@@ -141,6 +141,9 @@ def test_dir_stride_fields_are_validated_without_gpu(L):
     # k_chunk (chunked scan): 0 / 1 = global scan, > 1 accepted, negative refused
     assert call(k_chunk=0) == 0 and call(k_chunk=1) == 0 and call(k_chunk=5) == 0
     assert call(k_chunk=-1) == 1 and b"k_chunk" in L.gspn_last_error()
+    # flags: GSPN_FLAG_W3_LOGITS accepted, unknown bits refused
+    assert call(flags=1) == 0
+    assert call(flags=2) == 1 and b"flags" in L.gspn_last_error()
     # the binding's helper: names -> strides
     assert bd._strides(("w3",)) == {"dir_stride_w3": 0, "dir_stride_lambda": bd.DIR_STRIDE_DENSE, "dir_stride_u": bd.DIR_STRIDE_DENSE}
     with pytest.raises(ValueError):

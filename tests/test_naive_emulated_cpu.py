@@ -40,8 +40,8 @@ def emu():
         os.replace(LIB + ".tmp", LIB)
     L = ctypes.CDLL(LIB)
     vp, ci, cu = ctypes.c_void_p, ctypes.c_int, ctypes.c_uint
-    L.emu_naive_fwd.argtypes = [vp] * 6 + [ci] * 5 + [cu, cu, ci, ci]
-    L.emu_naive_bwd.argtypes = [vp] * 11 + [ci] * 5 + [cu, cu, ci, ci]
+    L.emu_naive_fwd.argtypes = [vp] * 6 + [ci] * 5 + [cu, cu, ci, cu, ci]
+    L.emu_naive_bwd.argtypes = [vp] * 11 + [ci] * 5 + [cu, cu, ci, cu, ci]
     return L
 
 
@@ -61,16 +61,16 @@ def ptr(a):
     return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
 
 
-def run_fwd(L, cfg, dtype, t, shared=(), k_chunk=0):
+def run_fwd(L, cfg, dtype, t, shared=(), k_chunk=0, flags=0):
     d = {k: to_dev(v[0] if k in shared else v) for k, v in t.items()}
     y = np.full_like(d["x"], 0x7fc1 if dtype == "bf16" else np.nan)
     rc = L.emu_naive_fwd(ptr(d["x"]), ptr(d["w3"]), ptr(d["lam"]), ptr(d["u"]), ptr(d.get("h0")), ptr(y), cfg.B, cfg.C, cfg.H,
-                         cfg.W, cfg.G, cfg.dir_mask, sum(SHARED_BITS[k] for k in shared), k_chunk, 0 if dtype == "f32" else 1)
+                         cfg.W, cfg.G, cfg.dir_mask, sum(SHARED_BITS[k] for k in shared), k_chunk, flags, 0 if dtype == "f32" else 1)
     assert rc == 0
     return from_dev(y, dtype)
 
 
-def run_bwd(L, cfg, dtype, t, shared=(), k_chunk=0, need=("dx", "dlambda", "du", "dw3", "dh0")):
+def run_bwd(L, cfg, dtype, t, shared=(), k_chunk=0, need=("dx", "dlambda", "du", "dw3", "dh0"), flags=0):
     d = {k: to_dev(v[0] if k in shared else v) for k, v in t.items()}
     full = {k: to_dev(v) for k, v in t.items()}
     st = full["x"].dtype
@@ -81,7 +81,7 @@ def run_bwd(L, cfg, dtype, t, shared=(), k_chunk=0, need=("dx", "dlambda", "du",
     g = lambda k: ptr(out.get(k))
     rc = L.emu_naive_bwd(ptr(d["x"]), ptr(d["w3"]), ptr(d["lam"]), ptr(d["u"]), ptr(d.get("h0")), ptr(d["dy"]), g("dx"), g("dlambda"),
                          g("du"), g("dw3"), g("dh0"), cfg.B, cfg.C, cfg.H, cfg.W, cfg.G, cfg.dir_mask,
-                         sum(SHARED_BITS[k] for k in shared), k_chunk, 0 if dtype == "f32" else 1)
+                         sum(SHARED_BITS[k] for k in shared), k_chunk, flags, 0 if dtype == "f32" else 1)
     assert rc == 0
     return {k: from_dev(v, dtype) for k, v in out.items()}
 
@@ -153,6 +153,41 @@ def test_chunked_scan_emulated(emu, k_chunk, dtype):
             r = pu.gate(g[k], go[k], Ag[k], dtype)
             assert r["ok"], (shape, mask, k, r)
         np.testing.assert_array_equal(run_fwd(emu, cfg, dtype, t, k_chunk=1), run_fwd(emu, cfg, dtype, t))
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_logits_in_the_load_path_emulated(emu, dtype):
+    """GSPN_FLAG_W3_LOGITS: Eq. 3 where the taps are loaded, its adjoint where dw3 leaves; against the composition of the
+    oracle's normalize / fwd / bwd / normalize_bwd.  Also with one shared logit slab and with k_chunk (flags compose)."""
+    for shape, mask in [((2, 4, 8, 8, 2), 15), ((1, 2, 13, 17, 1), 15), ((1, 4, 10, 9, 2), 6), ((1, 2, 1, 12, 1), 15)]:
+        cfg = gi.small_config("emul", *shape, dir_mask=mask, seed=127, backward=True)
+        t = gi.make_inputs(cfg, dtype, device="cpu", with_dy=True, with_h0=True)
+        wt = gi.make_logits(cfg, dtype)["wt"]
+        tl = dict(t, w3=wt)
+        yo, A, go, Ag = pu.oracle_logits(t, wt, cfg)
+        r = pu.gate(run_fwd(emu, cfg, dtype, tl, flags=1), yo, A, dtype)
+        assert r["ok"], (shape, mask, r)
+        g = run_bwd(emu, cfg, dtype, tl, flags=1)
+        for k in go:
+            r = pu.gate(g[k], go[k], Ag[k], dtype)
+            assert r["ok"], (shape, mask, k, r)
+    # one shared logit slab: the same slab normalised per direction (the in-grid taps differ between the axes)
+    cfg = gi.small_config("emul2", 1, 4, 9, 11, 2, dir_mask=15, seed=128, backward=True)
+    t = gi.make_inputs(cfg, "f32", device="cpu", with_dy=True)
+    wt = gi.make_logits(cfg, "f32")["wt"]
+    rep = wt[:1].expand(cfg.D, *wt.shape[1:]).contiguous()
+    yo, A, go, Ag = pu.oracle_logits(t, rep, cfg)
+    tl = dict(t, w3=wt)
+    assert pu.gate(run_fwd(emu, cfg, "f32", tl, shared=("w3",), flags=1), yo, A, "f32")["ok"]
+    g = run_bwd(emu, cfg, "f32", tl, shared=("w3",), flags=1)
+    for k in go:
+        assert pu.gate(g[k], go[k], Ag[k], "f32")["ok"], k
+    # with bands: Eq. 3 then the chunked scan
+    n = {k: pu.np64(v) for k, v in t.items()}
+    w3 = orc.normalize(pu.np64(wt), 15)
+    yo = orc.fwd_chunked(n["x"], w3, n["lam"], n["u"], cfg.G, 15, 3)
+    A = orc.fwd_chunked_magnitude(n["x"], w3, n["lam"], n["u"], cfg.G, 15, 3)
+    assert pu.gate(run_fwd(emu, cfg, "f32", tl, k_chunk=3, flags=1), yo, A, "f32")["ok"]
 
 
 def test_optional_outputs_emulated(emu):

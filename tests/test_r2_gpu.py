@@ -374,3 +374,34 @@ def test_chunked_scan_matches_the_oracle(dtype, k_chunk):
     with pytest.raises(gspn.GspnError) as ei:
         gspn.gspn_scan_fwd(d["x"], d["w3"], d["lam"], d["u"], cfg.G, mask, k_chunk=2, impl=gspn.IMPL_CHAIN)
     assert ei.value.status == 2
+
+
+# ---------------------------------------------------------------------------------- logits in the load path (second half)
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_logits_in_the_load_path(dtype):
+    """GSPN_FLAG_W3_LOGITS: `w3` holds raw logits, Eq. 3 is applied where the taps are loaded (normalised taps never written
+    to memory), and the backward writes the gradient of the logits.  Oracle: normalize -> fwd, bwd -> normalize_bwd in fp64
+    (tests/parity_util.oracle_logits).  Also against the two-kernel route (gspn_normalize_fwd, then the scan) in fp32,
+    where both keep full-precision taps."""
+    for shape, mask in [((2, 4, 16, 16, 2), 15), ((1, 4, 37, 41, 2), 15), ((2, 2, 27, 27, 1), 6), ((1, 2, 70, 33, 1), 9)]:
+        cfg = gi.small_config("lgt", *shape, dir_mask=mask, seed=131, backward=True)
+        t = gi.make_inputs(cfg, dtype, device="cpu", with_dy=True, with_h0=True)
+        wt = gi.make_logits(cfg, dtype)["wt"]
+        d = {k: v.cuda() for k, v in t.items()}
+        wd = wt.cuda()
+        yo, A, go, Ag = pu.oracle_logits(t, wt, cfg)
+        y = gspn.gspn_scan_fwd(d["x"], wd, d["lam"], d["u"], cfg.G, mask, h0=d["h0"], w3_logits=True)
+        assert gspn.gspn_last_variant() == "naive_fwd"
+        r = pu.gate(pu.np64(y), yo, A, dtype)
+        assert r["ok"], (shape, mask, r)
+        g = gspn.gspn_scan_bwd(d["x"], wd, d["lam"], d["u"], d["dy"], cfg.G, mask, h0=d["h0"], w3_logits=True)
+        for k in ("dx", "dlambda", "du", "dw3", "dh0"):
+            r = pu.gate(pu.np64(g[k]), go[k], Ag[k], dtype)
+            assert r["ok"], (shape, mask, k, r)
+        if dtype == "f32":      # two-kernel route: normalise into fp32 taps, then the same naive scan
+            w3 = gspn.gspn_normalize_fwd(wd, mask)
+            y2 = gspn.gspn_scan_fwd(d["x"], w3, d["lam"], d["u"], cfg.G, mask, h0=d["h0"], impl=gspn.IMPL_NAIVE)
+            assert pu.gate(pu.np64(y2), yo, A, dtype)["ok"]
+    with pytest.raises(gspn.GspnError) as ei:
+        gspn.gspn_scan_fwd(d["x"], wd, d["lam"], d["u"], cfg.G, mask, w3_logits=True, impl=gspn.IMPL_CHAIN)
+    assert ei.value.status == 2
