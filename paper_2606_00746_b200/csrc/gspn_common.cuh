@@ -76,4 +76,14 @@ struct LaunchInfo {
 
 constexpr int kMaxSmemOptin = 227 * 1024;   // B200: 227 KB usable shared memory per CTA
 
+// A kernel launch: the CUDA launch statement -- or, under tests/emu only (GSPN_EMU), the host emulation that runs the
+// blocks one after another with host threads (the launchers are then checked together with their kernels: shared-memory
+// layout, tensor maps, grid).
+#ifdef GSPN_EMU
+#define GSPN_LAUNCH(kern, grid, block, smem_bytes, stream, ...) \
+    (void)emu::launch(dim3(grid), dim3(block), GSPN_EMU_SMEM, (size_t)(smem_bytes), [&] { kern(__VA_ARGS__); })
+#else
+#define GSPN_LAUNCH(kern, grid, block, smem_bytes, stream, ...) kern<<<grid, block, smem_bytes, stream>>>(__VA_ARGS__)
+#endif
+
 }  // namespace gspn

@@ -14,8 +14,15 @@
 
 #include "gspn_common.cuh"
 
+// GSPN_EMU is defined by tests/emu only: the PTX wrappers below are then replaced by host stand-ins of the same names
+// (tests/emu/emu_ptx.h), so that the kernels written on top of them can be run, and their protocols checked, without a GPU.
+#ifdef GSPN_EMU
+#include "emu_ptx.h"
+#endif
+
 namespace gspn {
 
+#ifndef GSPN_EMU
 // ---- shared-memory addresses / mbarriers -----------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
@@ -72,6 +79,7 @@ __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* m) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(m) : "memory");
 }
+#endif  // GSPN_EMU
 
 // ---- storage vectors ---------------------------------------------------------------------------
 // NB bytes (4, 8 or 16) of storage type ST read from shared memory and widened to fp32.
@@ -152,8 +160,10 @@ template <int N> __device__ __forceinline__ void stf(float* p, const float (&f)[
 // ---- host: tensor maps --------------------------------------------------------------------------
 // Encodes a tiled, unswizzled tensor map over `rank` dimensions (dims[0] is the contiguous one,
 // strides_bytes[i] is the stride of dims[i+1]).  Returns false and sets the library error on failure.
+#ifndef GSPN_EMU
 bool encode_tensor_map(CUtensorMap* out, int es, void* base, int rank, const uint64_t* dims,
                        const uint64_t* strides_bytes, const uint32_t* box, int swizzle32 = 0);
+#endif
 
 static inline int round_up_int(int v, int m) { return (v + m - 1) / m * m; }
 

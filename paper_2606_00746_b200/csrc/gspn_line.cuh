@@ -51,6 +51,7 @@ template <typename ST> __device__ __forceinline__ float line_elem(const uint32_t
     else return (e & 1) ? __uint_as_float(w[e >> 1] & 0xffff0000u) : __uint_as_float(w[e >> 1] << 16);
 }
 
+#ifndef GSPN_EMU      // (tests/emu/emu_ptx.h stands in for the PTX wrappers, see gspn_fused.cuh)
 // spinning wait (mbarrier.test_wait never suspends the thread)
 __device__ __forceinline__ void mbar_wait_spin(uint64_t* b, uint32_t parity) {
     asm volatile(
@@ -122,6 +123,7 @@ __device__ __forceinline__ void tm_alloc(uint32_t* slot, uint32_t cols) {
 __device__ __forceinline__ void tm_dealloc(uint32_t base, uint32_t cols) {
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(base), "r"(cols) : "memory");
 }
+#endif  // GSPN_EMU
 // the two warps of a channel meet: tensor-memory writes of one are visible to the other afterwards
 __device__ __forceinline__ void tm_pair_sync(int id) {
     tm_wait_st();
@@ -131,6 +133,7 @@ __device__ __forceinline__ void tm_pair_sync(int id) {
 }
 
 // ---- TMA stores shared -> global (tiled), bulk-group completion --------------------------------------------------
+#ifndef GSPN_EMU
 __device__ __forceinline__ void tma_store_3d(const CUtensorMap* m, const void* src, int c0, int c1, int c2) {
     asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];"
                  ::"l"(m), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2) : "memory");
@@ -156,6 +159,18 @@ __device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* m, int
         ::"r"(smem_u32(dst)), "l"(m), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
         : "memory");
 }
+// fma.rn.f32.bf16 (SASS FHFMA.BF16): c + a * b with a, b the low or the high bf16 half of a 32-bit word, no widening
+__device__ __forceinline__ float fma_bf16_half(uint32_t a, uint32_t b, bool high, float c) {
+    float d;
+    if (high)
+        asm("{ .reg .b16 al, ah, bl, bh;\n mov.b32 {al, ah}, %1;\n mov.b32 {bl, bh}, %2;\n fma.rn.f32.bf16 %0, ah, bh, %3; }"
+            : "=f"(d) : "r"(a), "r"(b), "f"(c));
+    else
+        asm("{ .reg .b16 al, ah, bl, bh;\n mov.b32 {al, ah}, %1;\n mov.b32 {bl, bh}, %2;\n fma.rn.f32.bf16 %0, al, bl, %3; }"
+            : "=f"(d) : "r"(a), "r"(b), "f"(c));
+    return d;
+}
+#endif  // GSPN_EMU
 
 // raw storage words of P elements (lambda and x are multiplied without widening: one FHFMA.BF16 per position)
 template <typename ST, int P> struct LineRaw { uint32_t w[(P * sizeof(ST) + 3) / 4]; };
@@ -168,14 +183,7 @@ template <typename ST> __device__ __forceinline__ float line_fma_raw(const uint3
     if constexpr (sizeof(ST) == 4) {
         return fmaf(__uint_as_float(a[k]), __uint_as_float(b[k]), c);
     } else {
-        float d;
-        if (k & 1)
-            asm("{ .reg .b16 al, ah, bl, bh;\n mov.b32 {al, ah}, %1;\n mov.b32 {bl, bh}, %2;\n fma.rn.f32.bf16 %0, ah, bh, %3; }"
-                : "=f"(d) : "r"(a[k >> 1]), "r"(b[k >> 1]), "f"(c));
-        else
-            asm("{ .reg .b16 al, ah, bl, bh;\n mov.b32 {al, ah}, %1;\n mov.b32 {bl, bh}, %2;\n fma.rn.f32.bf16 %0, al, bl, %3; }"
-                : "=f"(d) : "r"(a[k >> 1]), "r"(b[k >> 1]), "f"(c));
-        return d;
+        return fma_bf16_half(a[k >> 1], b[k >> 1], (k & 1) != 0, c);      // k is a compile-time constant after unrolling
     }
 }
 

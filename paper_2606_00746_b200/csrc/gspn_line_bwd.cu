@@ -833,7 +833,7 @@ static int line_bwd_run(const BwdArgs<ST>& a, cudaStream_t st) {
     auto kern = line_bwd_kernel<ST, NC, P>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("line bwd: cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return GSPN_ECUDA; }
-    kern<<<sh.B * sh.G, (NC + 1) * 32, off, st>>>(mv, mh, prm);
+    GSPN_LAUNCH(kern, sh.B * sh.G, (NC + 1) * 32, off, st, mv, mh, prm);
     e = cudaGetLastError();
     if (e != cudaSuccess) { set_error("line bwd: launch failed: %s", cudaGetErrorString(e)); return GSPN_ECUDA; }
     return GSPN_OK;

@@ -28,7 +28,11 @@ namespace {
 #define mbar_wait mbar_wait_spin
 #endif
 
+#ifndef GSPN_EMU
 __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#else
+inline unsigned long long gtime() { return 0; }
+#endif
 struct LineFwdParams {
     int B, C, H, W, G, cg;
     unsigned mask;
@@ -79,7 +83,7 @@ __device__ __forceinline__ void line_zero_edge_taps_h(unsigned char* sb, uint32_
 }
 // generic-proxy writes to a stage are ordered before the TMA writes that refill it
 __device__ __forceinline__ void line_release_stage(uint64_t* empty_bar, int lane) {
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    fence_proxy_async();
     __syncwarp();
     if (lane == 0) mbar_arrive(empty_bar);
 }
@@ -550,7 +554,7 @@ static int line_fwd_run(const FwdArgs<ST>& a, cudaStream_t st) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("line fwd: cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return GSPN_ECUDA; }
     const int items = sh.B * sh.G * (sh.cg() / NC);
-    kern<<<items, 320, smem, st>>>(m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], prm);
+    GSPN_LAUNCH(kern, items, 320, smem, st, m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], prm);
     e = cudaGetLastError();
     if (e != cudaSuccess) { set_error("line fwd: launch failed: %s", cudaGetErrorString(e)); return GSPN_ECUDA; }
     return GSPN_OK;

@@ -1,38 +1,20 @@
 // naive_emu.cpp -- TEST ONLY.  Runs the DEVICE code of the naive kernels (paper_2606_00746_b200/csrc/gspn_naive.cuh, the
 // file the library compiles with nvcc) on the host: compiled with g++ against tests/emu/shim (a few lines standing in for
-// the CUDA headers), one thread block at a time, its threads as host threads, __syncthreads as a std::barrier.  It exists
+// the CUDA headers) and tests/emu/emu_rt.h: one thread block at a time, its threads as host threads.  It exists
 // so that a change to those kernels can be checked against the oracle on a machine without a GPU
 // (tests/test_naive_emulated_cpu.py).  It is not a CPU path of the library: nothing under paper_2606_00746_b200/ knows
 // about it, and it emulates nothing but the naive kernels' plain threadIdx / __syncthreads / shared-memory model.
-#include <thread>
-#include <vector>
+#include <cuda_runtime.h>
 
 #include "gspn_naive.cuh"
 
-namespace emu {
-thread_local uint3 tid;
-uint3 bid;
-dim3 bdim, gdim;
-std::barrier<>* block_barrier;
-}  // namespace emu
-
 namespace gspn {
-float smem[1 << 20];      // dynamic shared memory of the running block (4 MB: far above the 227 KB a real CTA has)
+alignas(16) float smem[1 << 20];      // dynamic shared memory of the running block (4 MB: far above the 227 KB a real CTA has)
 }
 
 template <typename F>
 static void run_grid(unsigned blocks, unsigned threads, F kernel) {
-    emu::gdim.x = blocks;
-    emu::bdim.x = threads;
-    for (unsigned b = 0; b < blocks; ++b) {
-        emu::bid = uint3{b, 0, 0};
-        std::barrier<> bar((std::ptrdiff_t)threads);
-        emu::block_barrier = &bar;
-        std::vector<std::thread> pool;
-        for (unsigned t = 0; t < threads; ++t)
-            pool.emplace_back([=] { emu::tid = uint3{t, 0, 0}; kernel(); });
-        for (auto& th : pool) th.join();
-    }
+    emu::launch(dim3(blocks), dim3(threads), reinterpret_cast<unsigned char*>(gspn::smem), sizeof(gspn::smem), kernel);
 }
 
 static int round_up32(int v) { return (v + 31) / 32 * 32; }
@@ -42,7 +24,7 @@ static int fwd_t(const void* x, const void* w3, const void* lam, const void* u, 
     gspn::FwdArgs<ST> a{(const ST*)x, (const ST*)w3, (const ST*)lam, (const ST*)u, (const ST*)h0, (ST*)y, sh};
     if ((sh.plane() + 2 * (sh.Lmax() + 2)) > sizeof(gspn::smem) / 4) return 2;
     run_grid(sh.B * sh.C, round_up32(sh.Lmax()), [=] { gspn::naive_fwd_kernel<ST>(a); });      // grid / block of naive_fwd_launch
-    return 0;
+    return emu::failed.load() ? 5 : 0;
 }
 
 template <typename ST>
@@ -56,7 +38,7 @@ static int bwd_t(const void* x, const void* w3, const void* lam, const void* u, 
         run_grid(sh.B * sh.C, round_up32(sh.Lmax()), [=] { gspn::naive_bwd_main_kernel<ST>(a); });
     if (a.dw3)
         run_grid(sh.D() * sh.B * sh.G, round_up32(sh.Lmax()), [=] { gspn::naive_bwd_dw_kernel<ST>(a); });
-    return 0;
+    return emu::failed.load() ? 5 : 0;
 }
 
 extern "C" {

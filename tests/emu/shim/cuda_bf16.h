@@ -3,6 +3,7 @@
 #include <cstdint>
 #include <cstring>
 struct __nv_bfloat16 { unsigned short x; };
+struct __nv_bfloat162 { __nv_bfloat16 x, y; };
 inline __nv_bfloat16 __float2bfloat16_rn(float f) {
     uint32_t v; std::memcpy(&v, &f, 4);
     __nv_bfloat16 r;
@@ -11,3 +12,4 @@ inline __nv_bfloat16 __float2bfloat16_rn(float f) {
     r.x = (unsigned short)(v >> 16);
     return r;
 }
+inline __nv_bfloat162 __floats2bfloat162_rn(float a, float b) { return __nv_bfloat162{__float2bfloat16_rn(a), __float2bfloat16_rn(b)}; }

@@ -31,10 +31,10 @@ SHARED_BITS = {"w3": 1, "lam": 2, "u": 4}
 
 @pytest.fixture(scope="module")
 def emu():
-    srcs = [os.path.join(EMU, "naive_emu.cpp"), os.path.join(EMU, "shim", "cuda_runtime.h"), os.path.join(EMU, "shim", "cuda_bf16.h"),
+    srcs = [os.path.join(EMU, "naive_emu.cpp"), os.path.join(EMU, "shim", "cuda_runtime.h"), os.path.join(EMU, "shim", "cuda_bf16.h"), os.path.join(EMU, "emu_rt.h"),
             os.path.join(CSRC, "gspn_naive.cuh"), os.path.join(CSRC, "gspn_common.cuh")]
     if not os.path.exists(LIB) or os.path.getmtime(LIB) < max(os.path.getmtime(s) for s in srcs):
-        cmd = ["g++", "-std=c++20", "-O1", "-pthread", "-fPIC", "-shared", "-ffp-contract=off", "-I", os.path.join(EMU, "shim"),
+        cmd = ["g++", "-std=c++20", "-O1", "-pthread", "-fPIC", "-shared", "-ffp-contract=off", "-I", EMU, "-I", os.path.join(EMU, "shim"),
                "-I", CSRC, "-o", LIB + ".tmp", srcs[0]]
         subprocess.run(cmd, check=True)
         os.replace(LIB + ".tmp", LIB)
