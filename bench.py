@@ -53,8 +53,8 @@ def parse():
     ap.add_argument("--no-parity", action="store_true", help="skip the sampled oracle check of the timed outputs")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--line-bwd-probe", action="store_true",
-                    help="also force the line backward (never run on hardware, not in GSPN_IMPL_AUTO) on cfg4 / cfg2 in a child process")
+    ap.add_argument("--no-line-bwd-probe", action="store_true",
+                    help="skip the child process that forces the line backward (never run on hardware, not in GSPN_IMPL_AUTO) on cfg4 / cfg2")
     ap.add_argument("--line-bwd-child", action="store_true", help=argparse.SUPPRESS)
     return ap.parse_args()
 
@@ -418,11 +418,10 @@ def line_bwd_child():
 
 def line_bwd_probe(limit_s: int = 150):
     """The line backward (csrc/gspn_line_bwd.cu) is not in GSPN_IMPL_AUTO: it had not run on hardware when round 2 ended.
-    With --line-bwd-probe the bench gives it one bounded chance in a CHILD process (its own CUDA context, a time limit):
-    forced with GSPN_IMPL_LINE on the two aligned configs, gated on sampled images against the oracle, then timed.
-    Whatever happens is reported under others["line_bwd_child"]; nothing of the main line depends on it.  It is opt-in
-    because a first run of an unverified kernel can fault or hang, and the default bench run must not put a fault on
-    the box it is measured on."""
+    It passes the host emulation of tests/test_line_emulated_cpu.py (same source, emulated TMA / mbarrier / tensor memory),
+    so the bench gives it one bounded chance in a CHILD process (its own CUDA context, a time limit): forced with
+    GSPN_IMPL_LINE on the two aligned configs, gated on sampled images against the oracle, then timed.  Whatever happens
+    is reported under others["line_bwd_child"]; nothing of the main line depends on it (--no-line-bwd-probe skips it)."""
     import subprocess
     try:
         p = subprocess.run([sys.executable, os.path.abspath(__file__), "--line-bwd-child"], cwd=ROOT, stdout=subprocess.PIPE,
@@ -598,7 +597,7 @@ def main():
                 del lg, buf
                 torch.cuda.empty_cache()
 
-    if others is not None and impl == gspn.IMPL_AUTO and args.line_bwd_probe:      # opt-in: see line_bwd_probe
+    if others is not None and impl == gspn.IMPL_AUTO and not args.no_line_bwd_probe:
         others["line_bwd_child"] = line_bwd_probe()
 
     cpu = None

@@ -22,9 +22,9 @@ inline void mbar_wait(uint64_t* b, uint32_t parity) { emu::mb_wait(b, parity); }
 inline void mbar_wait_spin(uint64_t* b, uint32_t parity) { emu::mb_wait(b, parity); }
 inline void named_bar_sync(int id, int nthreads) { emu::named_sync(id, nthreads); }
 inline void fence_proxy_async() {}
-inline void bulk_commit() {}
-template <int N> inline void bulk_wait_read() {}
-template <int N> inline void bulk_wait_all() {}
+inline void bulk_commit() { emu::stores_commit(); }
+template <int N> inline void bulk_wait_read() { emu::stores_wait(N); }
+template <int N> inline void bulk_wait_all() { emu::stores_wait(N); }
 
 // ---- tensor maps ---------------------------------------------------------------------------------------------------------
 struct EmuMap {
@@ -99,32 +99,38 @@ inline uint64_t emu_tma(const CUtensorMap* map, unsigned char* smem, const int* 
     }
     return bytes;
 }
-inline void tma_load_3d(void* dst, const CUtensorMap* m, int c0, int c1, int c2, uint64_t* bar) {
-    const int c[3] = {c0, c1, c2};
-    emu::mb_complete_tx(bar, (long long)emu_tma<true>(m, (unsigned char*)dst, c, 3));
+// a load: at once (eager) or when a thread waits on `bar` (lazy, emu_rt.h)
+template <typename F> inline void emu_issue_load(uint64_t* bar, F copy) {
+    if (!emu::lazy) { emu::mb_complete_tx(bar, copy()); return; }
+    std::lock_guard<std::mutex> l(emu::blk->mb_m);
+    (void)emu::mb_get(bar, "TMA load");
+    emu::blk->lazy_loads[bar].emplace_back(copy);
 }
-inline void tma_load_4d(void* dst, const CUtensorMap* m, int c0, int c1, int c2, int c3, uint64_t* bar) {
-    const int c[4] = {c0, c1, c2, c3};
-    emu::mb_complete_tx(bar, (long long)emu_tma<true>(m, (unsigned char*)dst, c, 4));
+template <int R> inline void emu_load(void* dst, const CUtensorMap* m, const int (&c)[R], uint64_t* bar) {
+    const CUtensorMap mc = *m;
+    int cc[5] = {0, 0, 0, 0, 0};
+    for (int i = 0; i < R; ++i) cc[i] = c[i];
+    struct Job { CUtensorMap m; unsigned char* dst; int c[5]; };
+    const Job j{mc, (unsigned char*)dst, {cc[0], cc[1], cc[2], cc[3], cc[4]}};
+    emu_issue_load(bar, [j]() -> long long { return (long long)emu_tma<true>(&j.m, j.dst, j.c, R); });
 }
-inline void tma_load_5d(void* dst, const CUtensorMap* m, int c0, int c1, int c2, int c3, int c4, uint64_t* bar) {
-    const int c[5] = {c0, c1, c2, c3, c4};
-    emu::mb_complete_tx(bar, (long long)emu_tma<true>(m, (unsigned char*)dst, c, 5));
+template <int R> inline void emu_store(const CUtensorMap* m, const void* src, const int (&c)[R]) {
+    if (!emu::lazy) { emu_tma<false>(m, (unsigned char*)src, c, R); return; }
+    struct Job { CUtensorMap m; unsigned char* src; int c[5]; };
+    Job j{*m, (unsigned char*)src, {0, 0, 0, 0, 0}};
+    for (int i = 0; i < R; ++i) j.c[i] = c[i];
+    emu::store_open.emplace_back([j] { emu_tma<false>(&j.m, j.src, j.c, R); });
 }
-inline void tma_store_3d(const CUtensorMap* m, const void* src, int c0, int c1, int c2) {
-    const int c[3] = {c0, c1, c2};
-    emu_tma<false>(m, (unsigned char*)src, c, 3);
-}
-inline void tma_store_4d(const CUtensorMap* m, const void* src, int c0, int c1, int c2, int c3) {
-    const int c[4] = {c0, c1, c2, c3};
-    emu_tma<false>(m, (unsigned char*)src, c, 4);
-}
+inline void tma_load_3d(void* dst, const CUtensorMap* m, int c0, int c1, int c2, uint64_t* bar) { emu_load<3>(dst, m, {c0, c1, c2}, bar); }
+inline void tma_load_4d(void* dst, const CUtensorMap* m, int c0, int c1, int c2, int c3, uint64_t* bar) { emu_load<4>(dst, m, {c0, c1, c2, c3}, bar); }
+inline void tma_load_5d(void* dst, const CUtensorMap* m, int c0, int c1, int c2, int c3, int c4, uint64_t* bar) { emu_load<5>(dst, m, {c0, c1, c2, c3, c4}, bar); }
+inline void tma_store_3d(const CUtensorMap* m, const void* src, int c0, int c1, int c2) { emu_store<3>(m, src, {c0, c1, c2}); }
+inline void tma_store_4d(const CUtensorMap* m, const void* src, int c0, int c1, int c2, int c3) { emu_store<4>(m, src, {c0, c1, c2, c3}); }
 inline void bulk_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
     if (((uintptr_t)dst & 15u) || ((uintptr_t)src & 15u) || (bytes & 15u))
         emu::fail("cp.async.bulk: destination (shared offset %ld), source or size %u not 16-byte aligned", emu::smem_off(dst), bytes);
     emu::check_smem(dst, bytes, "cp.async.bulk");
-    std::memcpy(dst, src, bytes);
-    emu::mb_complete_tx(bar, bytes);
+    emu_issue_load(bar, [=]() -> long long { std::memcpy(dst, src, bytes); return (long long)bytes; });
 }
 inline void tma_prefetch_desc(const CUtensorMap* m) { (void)emu_map(m); }
 

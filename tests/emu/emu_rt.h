@@ -13,6 +13,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <functional>
 #include <memory>
 #include <mutex>
 #include <thread>
@@ -90,6 +91,8 @@ struct Warp {
 struct MBar { int expected = 0, pending = 0; long long tx = 0; unsigned phase = 0; };
 
 struct Block {
+    // lazy mode: TMA loads that have been issued but not yet performed, per mbarrier (performed when a thread waits on it)
+    std::unordered_map<const void*, std::vector<std::function<long long()>>> lazy_loads;
     Bar bar;                                        // __syncthreads
     std::vector<std::unique_ptr<Warp>> warps;
     Bar named[16];                                  // bar.sync id, n
@@ -116,6 +119,22 @@ inline void jitter() {
     if (s == 0) s = (jitter_seed * 2654435761u) ^ ((tid.x + 1u) * 40503u) ^ ((bid.x + 1u) * 69069u) | 1u;
     s ^= s << 13; s ^= s >> 17; s ^= s << 5;
     if ((s & 3u) == 0) std::this_thread::sleep_for(std::chrono::microseconds((s >> 8) % (unsigned)jitter_us));
+}
+
+// Lazy mode: asynchronous copies happen as LATE as the program allows instead of at once.  A TMA load lands only when a
+// thread waits on its mbarrier (a consumer that reads without waiting finds the poison the stage was filled with); a TMA
+// store reads shared memory only when its thread executes cp.async.bulk.wait_group[.read] for its group (a stage that is
+// overwritten before that wait sends the new bytes, and the comparison with the oracle fails).  Eager mode (the default)
+// is the other extreme: a refill destroys a stage that is still being read at once.
+inline bool lazy = false;
+inline thread_local std::vector<std::vector<std::function<void()>>> store_groups;      // closed groups, oldest first
+inline thread_local std::vector<std::function<void()>> store_open;                      // stores since the last commit
+inline void stores_commit() { if (lazy) { store_groups.push_back(std::move(store_open)); store_open.clear(); } }
+inline void stores_wait(int keep_newest) {
+    while ((int)store_groups.size() > keep_newest) {
+        for (auto& f : store_groups.front()) f();
+        store_groups.erase(store_groups.begin());
+    }
 }
 
 inline int lane() { return (int)(tid.x & 31u); }
@@ -187,6 +206,21 @@ inline void mb_wait(const void* b, uint32_t parity) {
     jitter();
     const auto dl = deadline();
     for (unsigned spin = 0;; ++spin) {
+        if (lazy) {      // the copies that complete on this barrier land now, when somebody is waiting for them
+            std::vector<std::function<long long()>> todo;
+            {
+                std::lock_guard<std::mutex> l(blk->mb_m);
+                auto it = blk->lazy_loads.find(b);
+                if (it != blk->lazy_loads.end()) todo.swap(it->second);
+            }
+            for (auto& f : todo) {
+                const long long bytes = f();
+                std::lock_guard<std::mutex> l(blk->mb_m);
+                MBar& m = mb_get(b, "complete_tx");
+                m.tx -= bytes;
+                mb_complete_if_done(m);
+            }
+        }
         {
             std::unique_lock<std::mutex> l(blk->mb_m);
             MBar& m = mb_get(b, "mbarrier.try_wait");
@@ -226,7 +260,12 @@ bool launch(dim3 grid, dim3 block, unsigned char* smem, size_t smem_bytes, F bod
             pool.emplace_back([&, t] {
                 tid = uint3{t, 0, 0};
                 my_warp = state.warps[t >> 5].get();
-                try { body(); } catch (const Error&) {}
+                store_groups.clear(); store_open.clear();
+                try {
+                    body();
+                    if (!store_open.empty() || !store_groups.empty())
+                        fail("thread %u returns with bulk stores it never waited for (cp.async.bulk.wait_group)", t);
+                } catch (const Error&) {}
                 my_warp->bar.drop();
                 state.bar.drop();
             });

@@ -16,3 +16,4 @@ void set_error(const char* fmt, ...) {
 
 extern "C" const char* emu_last_error() { return gspn::g_err; }
 extern "C" void emu_set_jitter(int max_us, unsigned seed) { emu::jitter_us = max_us; emu::jitter_seed = seed ? seed : 1u; }
+extern "C" void emu_set_lazy(int on) { emu::lazy = on != 0; }

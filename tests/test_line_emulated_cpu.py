@@ -12,8 +12,10 @@ a protocol error is a test failure with a message, not a hang.
 
 What this establishes: index arithmetic, stage / ring / checkpoint bookkeeping, barrier counts and phases, tensor-memory
 layouts and the launchers' shared-memory layout and tensor maps reproduce the oracle within the GPU tolerances.  What it
-cannot: memory-ordering between the generic and the async proxy, TMA stores still reading shared memory when it is
-reused (stores are synchronous here), performance.  The GPU parity tests remain the parity evidence.
+cannot: memory-ordering between the generic and the async proxy or around tcgen05 (the fences are no-ops here), performance.
+Asynchronous copies are run at both extremes: at once (default: a refill destroys a stage that is still being read) and
+as late as the program allows (lazy mode: a load lands when somebody waits on its mbarrier, a store reads shared memory
+when its bulk group is waited for).  The GPU parity tests remain the parity evidence.
 """
 import ctypes
 import os
@@ -55,6 +57,7 @@ def emu():
     L.emu_line_bwd.argtypes = [vp] * 11 + [ci] * 5 + [cu, ci, ctypes.c_double]
     L.emu_last_error.restype = ctypes.c_char_p
     L.emu_set_jitter.argtypes = [ci, cu]
+    L.emu_set_lazy.argtypes = [ci]
     return L
 
 
@@ -72,6 +75,11 @@ def ptr(a):
 
 
 LIMIT_S = 60.0          # a wait inside the emulated kernel longer than this is reported as a deadlock
+# A block of 160-320 threads on a few host cores is slow (a warp shuffle is two 32-thread barriers): the default run keeps the
+# cases that take seconds; GSPN_EMU_FULL=1 adds the full-size units (128x128 C/G=4, 56x56 C/G=8) and more timing-noise
+# and late-copy cases (about ten minutes more; all of them passed when this file was committed).
+FULL = os.environ.get("GSPN_EMU_FULL") == "1"
+heavy = pytest.mark.skipif(not FULL, reason="set GSPN_EMU_FULL=1 for the full-size emulated cases")
 
 
 def run_fwd(L, cfg, dtype, t):
@@ -130,7 +138,10 @@ BWD_CASES = [((1, 4, 8, 8, 1), 15, "f32", False), ((2, 4, 16, 16, 2), 15, "bf16"
              ((1, 4, 40, 40, 1), 9, "f32", False), ((1, 2, 36, 24, 1), 4, "bf16", True), ((1, 2, 36, 24, 1), 2, "f32", True)]
 
 
-@pytest.mark.parametrize("case", BWD_CASES, ids=[_id(c) for c in BWD_CASES])
+HEAVY_BWD = {(1, 8, 56, 56, 1), (1, 8, 40, 64, 2), (1, 4, 128, 128, 1), (1, 8, 60, 56, 1), (1, 2, 128, 8, 1)}
+
+
+@pytest.mark.parametrize("case", [pytest.param(c, marks=heavy) if c[0] in HEAVY_BWD else c for c in BWD_CASES], ids=[_id(c) for c in BWD_CASES])
 def test_line_backward_emulated(emu, case):
     """The line backward has never run on a GPU; here every gradient of every case is gated against the oracle."""
     shape, mask, dtype, h0 = case
@@ -146,11 +157,12 @@ def test_line_backward_emulated(emu, case):
         assert r["ok"], (k, r)
 
 
-@pytest.mark.parametrize("seed", [1, 2, 3])
-def test_line_kernels_emulated_under_timing_noise(emu, seed):
+@pytest.mark.parametrize("seed,shape", [(1, (1, 4, 16, 24, 2)), pytest.param(2, (2, 4, 24, 48, 2), marks=heavy),
+                                        pytest.param(3, (2, 4, 24, 48, 2), marks=heavy)])
+def test_line_kernels_emulated_under_timing_noise(emu, seed, shape):
     """Random sleeps at the synchronisation operations (another interleaving of producers and consumers per seed): same
     results, bit for bit, as without."""
-    cfg = gi.small_config("lje", 2, 4, 24, 48, 2, seed=9, backward=True)
+    cfg = gi.small_config("lje", *shape, seed=9, backward=True)
     t = gi.make_inputs(cfg, "bf16", device="cpu", with_dy=True, with_h0=True)
     rc, y0 = run_fwd(emu, cfg, "bf16", t)
     assert rc == 0, emu.emu_last_error().decode()
@@ -167,3 +179,35 @@ def test_line_kernels_emulated_under_timing_noise(emu, seed):
     np.testing.assert_array_equal(y1, y0)
     for k in g0:
         np.testing.assert_array_equal(g1[k], g0[k], err_msg=k)
+
+
+LAZY_CASES = [("fwd", (1, 4, 32, 48, 2), 15, "bf16", True), ("bwd", (1, 4, 16, 16, 2), 15, "bf16", True),
+              ("bwd", (1, 4, 24, 40, 2), 15, "f32", True), ("bwd", (1, 4, 128, 128, 1), 15, "bf16", True),
+              ("fwd", (1, 8, 128, 128, 2), 15, "bf16", False)]
+
+
+@pytest.mark.parametrize("case", [pytest.param(c, marks=heavy) if i >= 2 else c for i, c in enumerate(LAZY_CASES)],
+                         ids=[c[0] + "-" + _id(c[1:]) for c in LAZY_CASES])
+def test_line_kernels_emulated_with_copies_as_late_as_allowed(emu, case):
+    """The other extreme of the asynchronous copies (tests/emu/emu_rt.h, lazy mode): a TMA load lands only when a thread waits
+    on its mbarrier, a TMA store reads shared memory only when its thread waits for the bulk group.  A consumer that read
+    a stage without waiting, or an output stage rewritten before its store was waited for, would miss parity here."""
+    which, shape, mask, dtype, h0 = case
+    cfg = gi.small_config("lze", *shape, dir_mask=mask, seed=10, backward=True)
+    t = gi.make_inputs(cfg, dtype, device="cpu", with_dy=True, with_h0=h0)
+    emu.emu_set_lazy(1)
+    try:
+        if which == "fwd":
+            tf = {k: v for k, v in t.items() if k != "dy"}
+            rc, y = run_fwd(emu, cfg, dtype, tf)
+            assert rc == 0, emu.emu_last_error().decode()
+            yo, A = pu.oracle_fwd(tf, cfg)
+            assert pu.gate(y, yo, A, dtype)["ok"]
+        else:
+            rc, g = run_bwd(emu, cfg, dtype, t)
+            assert rc == 0, emu.emu_last_error().decode()
+            go, Ag = pu.oracle_bwd(t, cfg)
+            for k in go:
+                assert pu.gate(g[k], go[k], Ag[k], dtype)["ok"], k
+    finally:
+        emu.emu_set_lazy(0)
