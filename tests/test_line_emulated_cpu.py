@@ -211,3 +211,57 @@ def test_line_kernels_emulated_with_copies_as_late_as_allowed(emu, case):
                 assert pu.gate(g[k], go[k], Ag[k], dtype)["ok"], k
     finally:
         emu.emu_set_lazy(0)
+
+
+def _poison_taps(w3: torch.Tensor, cfg) -> torch.Tensor:
+    """NaN in every tap whose neighbour lies outside the grid (include/gspn.h: such a tap is never used)."""
+    w = w3.clone()
+    for q, d in enumerate(gi.dir_list(cfg.dir_mask)):
+        if d < 2:
+            w[q, :, :, 0, :, 0] = float("nan"); w[q, :, :, 2, :, cfg.W - 1] = float("nan")
+        else:
+            w[q, :, :, 0, 0, :] = float("nan"); w[q, :, :, 2, cfg.H - 1, :] = float("nan")
+    return w
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_line_kernels_never_use_out_of_grid_taps_emulated(emu, dtype):
+    """DESIGN.md reading 3 for the line kernels: NaN stored in the out-of-grid taps changes no output bit, forward or
+    backward (the dw3 entries of those taps are written 0 either way)."""
+    for shape in [(1, 4, 16, 16, 2), (1, 2, 40, 24, 1)]:
+        cfg = gi.small_config("lpe", *shape, seed=11, backward=True)
+        t = gi.make_inputs(cfg, dtype, device="cpu", with_dy=True)
+        bad = dict(t, w3=_poison_taps(t["w3"], cfg))
+        tf, bf = ({k: v for k, v in d.items() if k != "dy"} for d in (t, bad))
+        rc0, y0 = run_fwd(emu, cfg, dtype, tf)
+        rc1, y1 = run_fwd(emu, cfg, dtype, bf)
+        assert rc0 == 0 and rc1 == 0, emu.emu_last_error().decode()
+        np.testing.assert_array_equal(y1, y0)
+        rc0, g0 = run_bwd(emu, cfg, dtype, t)
+        rc1, g1 = run_bwd(emu, cfg, dtype, bad)
+        assert rc0 == 0 and rc1 == 0, emu.emu_last_error().decode()
+        for k in g0:
+            np.testing.assert_array_equal(g1[k], g0[k], err_msg=f"{shape} {k}")
+
+
+def test_line_backward_optional_outputs_emulated(emu):
+    """Any subset of the gradients may be left out (NULL pointers): the others keep their bits."""
+    cfg = gi.small_config("loe", 1, 4, 24, 32, 2, seed=12, backward=True)
+    t = gi.make_inputs(cfg, "bf16", device="cpu", with_dy=True, with_h0=True)
+    d = {k: to_dev(v) for k, v in t.items()}
+    shapes = {"dx": d["x"].shape, "dlambda": d["lam"].shape, "du": d["u"].shape, "dw3": d["w3"].shape,
+              "dh0": (cfg.D, cfg.B, cfg.C, max(cfg.H, cfg.W))}
+
+    def run(need):
+        out = {k: np.full(shapes[k], 0x7fc1, dtype=np.uint16) for k in need}
+        g = lambda k: ptr(out.get(k))
+        rc = emu.emu_line_bwd(ptr(d["x"]), ptr(d["w3"]), ptr(d["lam"]), ptr(d["u"]), ptr(d["h0"]), ptr(d["dy"]), g("dx"), g("dlambda"),
+                              g("du"), g("dw3"), g("dh0"), cfg.B, cfg.C, cfg.H, cfg.W, cfg.G, cfg.dir_mask, 1, LIMIT_S)
+        assert rc == 0, emu.emu_last_error().decode()
+        return out
+
+    full = run(("dx", "dlambda", "du", "dw3", "dh0"))
+    for need in (("dx",), ("dw3",), ("du", "dh0"), ("dlambda", "dw3"), ("dh0",), ("dx", "dlambda", "du")):
+        part = run(need)
+        for k in need:
+            np.testing.assert_array_equal(part[k], full[k], err_msg=f"{need} {k}")
