@@ -287,7 +287,7 @@ static int launch_group(const BwdArgs<ST>& a, cudaStream_t st) {
     auto kern = group_bwd_kernel<ST, CG>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("fused bwd (group): cudaFuncSetAttribute(%zu B): %s", off, cudaGetErrorString(e)); return GSPN_ECUDA; }
-    kern<<<sh.B * sh.G, threads, off, st>>>(a, L);
+    GSPN_LAUNCH(kern, sh.B * sh.G, threads, off, st, a, L);
     e = cudaGetLastError();
     if (e != cudaSuccess) { set_error("fused bwd (group): launch failed: %s", cudaGetErrorString(e)); return GSPN_ECUDA; }
     return GSPN_OK;

@@ -12,4 +12,5 @@ inline __nv_bfloat16 __float2bfloat16_rn(float f) {
     r.x = (unsigned short)(v >> 16);
     return r;
 }
+inline unsigned short __bfloat16_as_ushort(__nv_bfloat16 v) { return v.x; }
 inline __nv_bfloat162 __floats2bfloat162_rn(float a, float b) { return __nv_bfloat162{__float2bfloat16_rn(a), __float2bfloat16_rn(b)}; }
