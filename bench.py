@@ -597,6 +597,24 @@ def main():
                 del lg, buf
                 torch.cuda.empty_cache()
 
+    if others is not None and impl == gspn.IMPL_AUTO:
+        # SURVEY 8(f) f2, first step (Table 1): the paper's large planes, forward, with whatever
+        # GSPN_IMPL_AUTO picks -- today the fall-back kernels (flat_fwd up to 256 positions, beyond that the naive kernel
+        # with its accumulator plane in the workspace): correct, far from the roofline, printed so that the distance shows
+        for B_, C_, L_ in ((16, 8, 256), (16, 8, 512), (16, 8, 1024)):
+            key = f"table1:{B_}x{C_}x{L_}x{L_}:bf16:fwd"
+            try:
+                oc = gi.small_config(f"table1_{L_}", B_, C_, L_, L_, 2, seed=7)
+                r, tt, yy, gg = time_config(gspn, torch, oc, "bf16", 3, 3, 1, impl, False)
+                fb = oc.fwd_bytes(2)
+                others[key] = {"variant": r["variant_fwd"], "ms": r["fwd_ms_mean"], "ms_min": r["fwd_ms_min"],
+                               "gbs": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9, "frac": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9 / peak,
+                               "pxch_per_s": oc.n / (r["fwd_ms_mean"] * 1e-3), "l2_flush": r["l2_flush"]}
+                del tt, yy, gg
+            except Exception as ex:      # noqa: BLE001 -- a row that cannot be measured says why
+                others[key] = {"variant": None, "error": repr(ex)[:200]}
+            torch.cuda.empty_cache()
+
     if others is not None and impl == gspn.IMPL_AUTO and not args.no_line_bwd_probe:
         others["line_bwd_child"] = line_bwd_probe()
 

@@ -167,6 +167,15 @@ typedef struct gspn_args {
      * chip to the fp32 group sum; one rounding).  Other bits: GSPN_EINVAL.  Served by the naive kernels only in this
      * version (as shared slabs above). */
     unsigned flags;
+    /* r2 (first step): caller-provided DEVICE scratch, 16-byte aligned, at least
+     * gspn_workspace_bytes(...) bytes, or NULL.  Needed only where no kernel holds the shape on chip: planes beyond shared
+     * memory (about 238 x 238 forward, 120 x 120 backward) with lines of at most 1024 positions are then served by the
+     * naive kernels with their plane-sized fp32 arrays (y or h / dx / dw3 accumulators) in this scratch, one slice per
+     * CTA.  The library never allocates it, never keeps it, and leaves its contents undefined; calls that share a
+     * workspace must not overlap on the GPU.  Without it such a shape reports GSPN_EWORKSPACE (the plain calls above
+     * pass none).  The fused kernels ignore it. */
+    void *workspace;
+    size_t workspace_bytes;
 } gspn_args_t;
 
 #define GSPN_FLAG_W3_LOGITS 1u
@@ -200,8 +209,10 @@ int gspn_scan_fwd_bwd_host(const void* x, const void* w3, const void* lambda, co
  * without a GPU).  A tensor of D slabs x B images x image_bytes; images [b0, b0 + bc) <-> a chunk laid out [D, bc]. */
 int gspn_debug_chunk_copy(void* chunk, void* host, size_t image_bytes, int D, int B, int b0, int bc, int to_chunk);
 
-/* Bytes of caller-provided scratch the device entry points need: always 0 in this
- * version (every intermediate lives on chip); kept so callers can be written once. */
+/* Bytes of caller-provided scratch (gspn_args_t.workspace) with which every shape of at most 1024 lines is served: 0
+ * where the fall-back kernel keeps its planes in shared memory (all five benchmark configs forward, cfg 2 / 3 / 5
+ * backward), else the fp32 planes it moves to global memory (forward B*C*H*W*4; backward the larger of 2*B*C*H*W*4 and
+ * 4*D*B*G*H*W*4).  An upper bound: a fused kernel that holds the shape does not touch the workspace. */
 size_t gspn_workspace_bytes(int B, int C, int H, int W, int G, unsigned dir_mask, int dtype, int is_bwd);
 
 /* Number of kernel launches the last successful call on this thread enqueued. */

@@ -45,7 +45,8 @@ class _Args(ctypes.Structure):
                 ("G", ctypes.c_int), ("dir_mask", ctypes.c_uint), ("dtype", ctypes.c_int),
                 ("impl", ctypes.c_int), ("stream", ctypes.c_void_p),
                 ("dir_stride_w3", ctypes.c_size_t), ("dir_stride_lambda", ctypes.c_size_t),
-                ("dir_stride_u", ctypes.c_size_t), ("k_chunk", ctypes.c_int), ("flags", ctypes.c_uint)]
+                ("dir_stride_u", ctypes.c_size_t), ("k_chunk", ctypes.c_int), ("flags", ctypes.c_uint),
+                ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t)]
 
 
 FLAG_W3_LOGITS = 1
@@ -131,6 +132,15 @@ def _stream(t):
     return ctypes.c_void_p(torch.cuda.current_stream(t.device).cuda_stream)
 
 
+def _workspace(x, B, C, H, W, G, dir_mask, is_bwd, impl):
+    """Scratch for planes beyond shared memory (gspn_args_t.workspace): allocated here, as every other tensor is, when
+    gspn_workspace_bytes asks for it and the call can reach the kernels that use it."""
+    if impl not in (IMPL_AUTO, IMPL_NAIVE):
+        return None
+    n = lib().gspn_workspace_bytes(B, C, H, W, G, dir_mask, _dtype_code(x), is_bwd)
+    return torch.empty(n, dtype=torch.uint8, device=x.device) if n else None
+
+
 def _shapes(x, G, dir_mask):
     B, C, H, W = x.shape
     D = _popcount(dir_mask)
@@ -151,15 +161,17 @@ def gspn_scan_fwd(x, w3, lam, u, G: int, dir_mask: int = DIR_ALL, h0=None, out=N
     _dev(lam, "lam", s_bc[1:] if "lam" in shared else s_bc, x); _dev(u, "u", s_bc[1:] if "u" in shared else s_bc, x)
     _dev(h0, "h0", s_h0, x)
     y = torch.empty_like(x) if out is None else _dev(out, "out", x.shape, x)
+    ws = _workspace(x, B, C, H, W, G, dir_mask, 0, impl)
     with torch.cuda.device(x.device):
-        if h0 is None and impl == IMPL_AUTO and not shared and k_chunk <= 1 and not w3_logits:
+        if h0 is None and impl == IMPL_AUTO and not shared and k_chunk <= 1 and not w3_logits and ws is None:
             rc = lib().gspn_scan_fwd(_p(x), _p(w3), _p(lam), _p(u), _p(y), B, C, H, W, G, dir_mask,
                                      _dtype_code(x), _stream(x))
         else:
             a = _Args(struct_size=ctypes.sizeof(_Args), x=x.data_ptr(), w3=w3.data_ptr(),
                       lam=lam.data_ptr(), u=u.data_ptr(), h0=None if h0 is None else h0.data_ptr(),
                       y=y.data_ptr(), B=B, C=C, H=H, W=W, G=G, dir_mask=dir_mask,
-                      dtype=_dtype_code(x), impl=impl,
+                      dtype=_dtype_code(x), impl=impl, workspace=None if ws is None else ws.data_ptr(),
+                      workspace_bytes=0 if ws is None else ws.numel(),
                       stream=torch.cuda.current_stream(x.device).cuda_stream, k_chunk=k_chunk, flags=FLAG_W3_LOGITS if w3_logits else 0, **_strides(shared))
             rc = lib().gspn_scan_fwd_ex(ctypes.byref(a))
     _check(rc)
@@ -181,8 +193,9 @@ def gspn_scan_bwd(x, w3, lam, u, dy, G: int, dir_mask: int = DIR_ALL, h0=None,
     shapes = {"dx": x.shape, "dlambda": s_bc, "du": s_bc, "dw3": s_w, "dh0": s_h0}
     out = {k: torch.empty(shapes[k], dtype=x.dtype, device=x.device) for k in need}
     g = lambda k: out[k].data_ptr() if k in out else None
+    ws = _workspace(x, B, C, H, W, G, dir_mask, 1, impl)
     with torch.cuda.device(x.device):
-        if h0 is None and impl == IMPL_AUTO and not shared and k_chunk <= 1 and not w3_logits:
+        if h0 is None and impl == IMPL_AUTO and not shared and k_chunk <= 1 and not w3_logits and ws is None:
             rc = lib().gspn_scan_bwd(_p(x), _p(w3), _p(lam), _p(u), _p(dy), g("dx"), g("dlambda"),
                                      g("du"), g("dw3"), g("dh0"), B, C, H, W, G, dir_mask,
                                      _dtype_code(x), _stream(x))
@@ -191,7 +204,8 @@ def gspn_scan_bwd(x, w3, lam, u, dy, G: int, dir_mask: int = DIR_ALL, h0=None,
                       lam=lam.data_ptr(), u=u.data_ptr(), h0=None if h0 is None else h0.data_ptr(),
                       dy=dy.data_ptr(), dx=g("dx"), dlambda=g("dlambda"), du=g("du"), dw3=g("dw3"),
                       dh0=g("dh0"), B=B, C=C, H=H, W=W, G=G, dir_mask=dir_mask,
-                      dtype=_dtype_code(x), impl=impl,
+                      dtype=_dtype_code(x), impl=impl, workspace=None if ws is None else ws.data_ptr(),
+                      workspace_bytes=0 if ws is None else ws.numel(),
                       stream=torch.cuda.current_stream(x.device).cuda_stream, k_chunk=k_chunk, flags=FLAG_W3_LOGITS if w3_logits else 0, **_strides(shared))
             rc = lib().gspn_scan_bwd_ex(ctypes.byref(a))
     _check(rc)

@@ -53,6 +53,8 @@ static unsigned shared_bits(const gspn_args_t* a) {
 }
 static int chunks(const gspn_args_t* a) { return a->struct_size == GSPN_ARGS_SIZE_R1 ? 0 : a->k_chunk; }
 static unsigned arg_flags(const gspn_args_t* a) { return a->struct_size == GSPN_ARGS_SIZE_R1 ? 0u : a->flags; }
+static float* arg_ws(const gspn_args_t* a) { return a->struct_size == GSPN_ARGS_SIZE_R1 ? nullptr : (float*)a->workspace; }
+static size_t arg_ws_bytes(const gspn_args_t* a) { return a->struct_size == GSPN_ARGS_SIZE_R1 || !a->workspace ? 0 : a->workspace_bytes; }
 
 template <typename ST>
 static int fwd_typed(const gspn_args_t* a) {
@@ -60,6 +62,7 @@ static int fwd_typed(const gspn_args_t* a) {
     f.x = (const ST*)a->x; f.w3 = (const ST*)a->w3; f.lam = (const ST*)a->lambda;
     f.u = (const ST*)a->u; f.h0 = (const ST*)a->h0; f.y = (ST*)a->y;
     f.sh = Shape{a->B, a->C, a->H, a->W, a->G, a->dir_mask, shared_bits(a), chunks(a), arg_flags(a)};
+    f.ws = arg_ws(a); f.ws_bytes = arg_ws_bytes(a);
     cudaStream_t st = (cudaStream_t)a->stream;
     LaunchInfo li{0, ""};
     int rc;
@@ -105,6 +108,7 @@ static int bwd_typed(const gspn_args_t* a) {
     f.dx = (ST*)a->dx; f.dlam = (ST*)a->dlambda; f.du = (ST*)a->du; f.dw3 = (ST*)a->dw3;
     f.dh0 = (ST*)a->dh0;
     f.sh = Shape{a->B, a->C, a->H, a->W, a->G, a->dir_mask, shared_bits(a), chunks(a), arg_flags(a)};
+    f.ws = arg_ws(a); f.ws_bytes = arg_ws_bytes(a);
     cudaStream_t st = (cudaStream_t)a->stream;
     LaunchInfo li{0, ""};
     int rc;
@@ -166,6 +170,7 @@ static int check_ex(const gspn_args_t* a) {
             }
         if (a->k_chunk < 0) { set_error("k_chunk=%d is negative (0 or 1 = the global scan)", a->k_chunk); return GSPN_EINVAL; }
         if (a->flags & ~GSPN_FLAG_W3_LOGITS) { set_error("flags=0x%x: unknown bit(s)", a->flags); return GSPN_EINVAL; }
+        if (a->workspace && !aligned16(a->workspace)) { set_error("pointer 'workspace' is not 16-byte aligned"); return GSPN_EALIGN; }
     }
     return GSPN_OK;
 }
@@ -458,7 +463,10 @@ done:
     return rc;
 }
 
-size_t gspn_workspace_bytes(int, int, int, int, int, unsigned, int, int) { return 0; }
+size_t gspn_workspace_bytes(int B, int C, int H, int W, int G, unsigned dir_mask, int dtype, int is_bwd) {
+    if (check_shape(B, C, H, W, G, dir_mask, dtype) != GSPN_OK) return 0;
+    return naive_workspace_bytes(Shape{B, C, H, W, G, dir_mask}, is_bwd != 0);
+}
 
 int gspn_last_launch_count(void) { return g_launches; }
 const char* gspn_last_variant(void) { return g_variant; }

@@ -59,6 +59,8 @@ struct FwdArgs {
     const ST *x, *w3, *lam, *u, *h0;
     ST* y;
     Shape sh;
+    float* ws;            // caller workspace (gspn_args_t.workspace) or NULL, and its size
+    size_t ws_bytes;
 };
 
 template <typename ST>
@@ -66,6 +68,8 @@ struct BwdArgs {
     const ST *x, *w3, *lam, *u, *h0, *dy;
     ST *dx, *dlam, *du, *dw3, *dh0;
     Shape sh;
+    float* ws;
+    size_t ws_bytes;
 };
 
 // launch results reported back to the C ABI

@@ -11,6 +11,8 @@ namespace gspn {
 // straight from global memory.  Reference GPU path for A/B runs; slow by design.
 template <typename ST> int naive_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
 template <typename ST> int naive_bwd_launch(const BwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);
+// bytes of caller workspace the naive kernels need for this shape (planes beyond shared memory), 0 if none
+size_t naive_workspace_bytes(const Shape& sh, bool bwd);
 
 // fused kernels: forward tile kernel (gspn_fused_fwd.cu), backward group kernel (gspn_group_bwd.cu).
 template <typename ST> int fused_fwd_launch(const FwdArgs<ST>& a, cudaStream_t st, LaunchInfo* li);

@@ -120,13 +120,18 @@ struct SlabIn {
     }
 };
 
+// (__launch_bounds__(1024): a block is as wide as the longest line, up to 1024 threads, so a thread may hold at most 64
+// registers; without the bound ptxas takes 86-120 and a launch with more than 544-736 threads fails.)
+// ws: NULL, or (large planes) global fp32 scratch that takes the place of the plane-sized shared-memory
+// arrays -- one slice per CTA, touched by that CTA only, every access of one element separated from the next by a
+// __syncthreads; shared memory then holds the two lines only
 template <typename ST>
-__global__ void naive_fwd_kernel(FwdArgs<ST> a) {
+__global__ void __launch_bounds__(1024) naive_fwd_kernel(FwdArgs<ST> a, float* ws) {
     extern __shared__ float smem[];
     const Shape sh = a.sh;
     const int H = sh.H, W = sh.W, plane = H * W, Lmax = sh.Lmax();
-    float* ysm = smem;
-    float* hbuf = smem + plane;
+    float* ysm = ws ? ws + (size_t)blockIdx.x * plane : smem;
+    float* hbuf = ws ? smem : smem + plane;
     const int bc = blockIdx.x, b = bc / sh.C, c = bc % sh.C, g = c / sh.cg();
     for (int o = threadIdx.x; o < plane; o += blockDim.x) ysm[o] = 0.f;
     __syncthreads();
@@ -228,13 +233,13 @@ __device__ void naive_pass_bwd(int dir, const ST* xp, const ST* wp, const ST* lp
 
 // grid B*C: dx (summed over directions on chip), dlambda, du, dh0
 template <typename ST>
-__global__ void naive_bwd_main_kernel(BwdArgs<ST> a) {
+__global__ void __launch_bounds__(1024) naive_bwd_main_kernel(BwdArgs<ST> a, float* ws) {
     extern __shared__ float smem[];
     const Shape sh = a.sh;
     const int H = sh.H, W = sh.W, plane = H * W, Lmax = sh.Lmax();
-    float* hall = smem;
-    float* dxs = smem + plane;
-    float* hbuf = dxs + plane;
+    float* hall = ws ? ws + (size_t)blockIdx.x * 2 * plane : smem;
+    float* dxs = hall + plane;
+    float* hbuf = ws ? smem : dxs + plane;
     float* ghs = hbuf + 2 * (Lmax + 2);
     const int bc = blockIdx.x, b = bc / sh.C, c = bc % sh.C, g = c / sh.cg();
     for (int o = threadIdx.x; o < plane; o += blockDim.x) dxs[o] = 0.f;
@@ -265,13 +270,13 @@ __global__ void naive_bwd_main_kernel(BwdArgs<ST> a) {
 
 // grid D*B*G: dw3 of one (direction slab, b, group), channels accumulated in ascending order
 template <typename ST>
-__global__ void naive_bwd_dw_kernel(BwdArgs<ST> a) {
+__global__ void __launch_bounds__(1024) naive_bwd_dw_kernel(BwdArgs<ST> a, float* ws) {
     extern __shared__ float smem[];
     const Shape sh = a.sh;
     const int H = sh.H, W = sh.W, plane = H * W, Lmax = sh.Lmax(), cg = sh.cg();
-    float* hall = smem;
-    float* dws = smem + plane;
-    float* hbuf = dws + 3 * plane;
+    float* hall = ws ? ws + (size_t)blockIdx.x * 4 * plane : smem;
+    float* dws = hall + plane;
+    float* hbuf = ws ? smem : dws + 3 * plane;
     float* ghs = hbuf + 2 * (Lmax + 2);
     const int q = blockIdx.x / (sh.B * sh.G);
     const int bg = blockIdx.x % (sh.B * sh.G), b = bg / sh.G, g = bg % sh.G;

@@ -36,6 +36,12 @@ def test_version_and_workspace(L):
     assert gspn.gspn_version() >= 100
     assert L.gspn_workspace_bytes(4, 256, 128, 128, 64, 15, 1, 0) == 0
     assert L.gspn_workspace_bytes(32, 128, 73, 73, 32, 15, 1, 1) == 0
+    # planes beyond shared memory: the fp32 planes the fall-back kernels move to the caller's workspace
+    assert L.gspn_workspace_bytes(16, 8, 1024, 1024, 2, 15, 1, 0) == 16 * 8 * 1024 * 1024 * 4
+    assert L.gspn_workspace_bytes(1, 2, 200, 200, 1, 15, 0, 0) == 0                       # 160 KB: still on chip
+    assert L.gspn_workspace_bytes(1, 2, 200, 200, 1, 15, 0, 1) == max(2 * 2, 4 * 4 * 1) * 200 * 200 * 4
+    assert L.gspn_workspace_bytes(4, 256, 128, 128, 64, 15, 1, 1) == 4 * 4 * 4 * 64 * 128 * 128 * 4   # cfg4 backward: the dw3 launch
+    assert L.gspn_workspace_bytes(1, 1, 2000, 8, 1, 15, 0, 0) == 0                        # lines beyond 1024: not held at all
 
 
 def test_argument_validation_without_gpu(L):

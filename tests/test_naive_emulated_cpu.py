@@ -40,8 +40,8 @@ def emu():
         os.replace(LIB + ".tmp", LIB)
     L = ctypes.CDLL(LIB)
     vp, ci, cu = ctypes.c_void_p, ctypes.c_int, ctypes.c_uint
-    L.emu_naive_fwd.argtypes = [vp] * 6 + [ci] * 5 + [cu, cu, ci, cu, ci]
-    L.emu_naive_bwd.argtypes = [vp] * 11 + [ci] * 5 + [cu, cu, ci, cu, ci]
+    L.emu_naive_fwd.argtypes = [vp] * 6 + [ci] * 5 + [cu, cu, ci, cu, ci, vp]
+    L.emu_naive_bwd.argtypes = [vp] * 11 + [ci] * 5 + [cu, cu, ci, cu, ci, vp]
     return L
 
 
@@ -61,16 +61,22 @@ def ptr(a):
     return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
 
 
-def run_fwd(L, cfg, dtype, t, shared=(), k_chunk=0, flags=0):
+def scratch(cfg, planes_per_cta, ctas):
+    """The large-plane mode's global scratch (csrc/gspn_naive.cu naive_workspace_bytes), NaN-filled; None = shared memory."""
+    return np.full(ctas * planes_per_cta * cfg.H * cfg.W, np.nan, dtype=np.float32)
+
+
+def run_fwd(L, cfg, dtype, t, shared=(), k_chunk=0, flags=0, ws=False):
     d = {k: to_dev(v[0] if k in shared else v) for k, v in t.items()}
     y = np.full_like(d["x"], 0x7fc1 if dtype == "bf16" else np.nan)
+    w = scratch(cfg, 1, cfg.B * cfg.C) if ws else None
     rc = L.emu_naive_fwd(ptr(d["x"]), ptr(d["w3"]), ptr(d["lam"]), ptr(d["u"]), ptr(d.get("h0")), ptr(y), cfg.B, cfg.C, cfg.H,
-                         cfg.W, cfg.G, cfg.dir_mask, sum(SHARED_BITS[k] for k in shared), k_chunk, flags, 0 if dtype == "f32" else 1)
+                         cfg.W, cfg.G, cfg.dir_mask, sum(SHARED_BITS[k] for k in shared), k_chunk, flags, 0 if dtype == "f32" else 1, ptr(w))
     assert rc == 0
     return from_dev(y, dtype)
 
 
-def run_bwd(L, cfg, dtype, t, shared=(), k_chunk=0, need=("dx", "dlambda", "du", "dw3", "dh0"), flags=0):
+def run_bwd(L, cfg, dtype, t, shared=(), k_chunk=0, need=("dx", "dlambda", "du", "dw3", "dh0"), flags=0, ws=False):
     d = {k: to_dev(v[0] if k in shared else v) for k, v in t.items()}
     full = {k: to_dev(v) for k, v in t.items()}
     st = full["x"].dtype
@@ -79,9 +85,10 @@ def run_bwd(L, cfg, dtype, t, shared=(), k_chunk=0, need=("dx", "dlambda", "du",
               "dh0": (cfg.D, cfg.B, cfg.C, max(cfg.H, cfg.W))}
     out = {k: np.full(shapes[k], fill, dtype=st) for k in need}
     g = lambda k: ptr(out.get(k))
+    w = scratch(cfg, 4, max(cfg.B * cfg.C, cfg.D * cfg.B * cfg.G)) if ws else None      # one buffer for both launches, as the launcher
     rc = L.emu_naive_bwd(ptr(d["x"]), ptr(d["w3"]), ptr(d["lam"]), ptr(d["u"]), ptr(d.get("h0")), ptr(d["dy"]), g("dx"), g("dlambda"),
                          g("du"), g("dw3"), g("dh0"), cfg.B, cfg.C, cfg.H, cfg.W, cfg.G, cfg.dir_mask,
-                         sum(SHARED_BITS[k] for k in shared), k_chunk, flags, 0 if dtype == "f32" else 1)
+                         sum(SHARED_BITS[k] for k in shared), k_chunk, flags, 0 if dtype == "f32" else 1, ptr(w))
     assert rc == 0
     return {k: from_dev(v, dtype) for k, v in out.items()}
 
@@ -188,6 +195,25 @@ def test_logits_in_the_load_path_emulated(emu, dtype):
     yo = orc.fwd_chunked(n["x"], w3, n["lam"], n["u"], cfg.G, 15, 3)
     A = orc.fwd_chunked_magnitude(n["x"], w3, n["lam"], n["u"], cfg.G, 15, 3)
     assert pu.gate(run_fwd(emu, cfg, "f32", tl, k_chunk=3, flags=1), yo, A, "f32")["ok"]
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_large_plane_mode_emulated(emu, dtype):
+    """SURVEY 8(f) f2, first step: the plane-sized fp32 arrays (y; h, dx; h, dw3) in a global workspace instead of shared
+    memory -- what the launchers switch to when a plane exceeds shared memory.  Forced here at small sizes (NaN-filled
+    scratch): same bits as the shared-memory mode, and the oracle's values."""
+    for shape, mask in [((2, 4, 9, 11, 2), 15), ((1, 2, 40, 7, 1), 6), ((1, 2, 6, 33, 2), 9)]:
+        cfg = gi.small_config("emuw", *shape, dir_mask=mask, seed=129, backward=True)
+        t = gi.make_inputs(cfg, dtype, device="cpu", with_dy=True, with_h0=True)
+        yo, A = pu.oracle_fwd(t, cfg)
+        y = run_fwd(emu, cfg, dtype, t, ws=True)
+        assert pu.gate(y, yo, A, dtype)["ok"], (shape, mask)
+        np.testing.assert_array_equal(y, run_fwd(emu, cfg, dtype, t))
+        go, Ag = pu.oracle_bwd(t, cfg)
+        g, g0 = run_bwd(emu, cfg, dtype, t, ws=True), run_bwd(emu, cfg, dtype, t)
+        for k in go:
+            assert pu.gate(g[k], go[k], Ag[k], dtype)["ok"], (shape, mask, k)
+            np.testing.assert_array_equal(g[k], g0[k], err_msg=k)
 
 
 def test_optional_outputs_emulated(emu):

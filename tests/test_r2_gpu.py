@@ -108,8 +108,9 @@ def test_auto_backward_on_the_aligned_benchmark_shapes(shape, dtype, record_prop
                      "memory; line_bwd holds it but is opt-in until it has run on hardware)")
     assert r["ok"], r
     record_property("variant", r["variant"])
-    if r["variant"] == "naive_bwd":
-        pytest.xfail("GSPN_IMPL_AUTO has no fused backward for this shape yet (line_bwd is opt-in until it has run on hardware)")
+    if r["variant"].startswith("naive_bwd"):
+        pytest.xfail("GSPN_IMPL_AUTO has no fused backward for this shape yet: it lands on " + r["variant"] +
+                     " (line_bwd holds the shape but stays out of AUTO until it has run on hardware)")
 
 
 # ---------------------------------------------------------------------------------- out-of-grid taps (hole f, reading 3)
@@ -404,4 +405,51 @@ def test_logits_in_the_load_path(dtype):
             assert pu.gate(pu.np64(y2), yo, A, dtype)["ok"]
     with pytest.raises(gspn.GspnError) as ei:
         gspn.gspn_scan_fwd(d["x"], wd, d["lam"], d["u"], cfg.G, mask, w3_logits=True, impl=gspn.IMPL_CHAIN)
+    assert ei.value.status == 2
+
+
+# ---------------------------------------------------------------------------------- large planes (first step)
+@pytest.mark.parametrize("shape,dtype", [((1, 2, 256, 256, 1), "bf16"), ((1, 2, 300, 260, 2), "f32"), ((1, 2, 1024, 1024, 1), "bf16"),
+                                         ((2, 2, 512, 64, 1), "f32")], ids=["256x256-bf16", "300x260-f32", "1024x1024-bf16", "512x64-f32"])
+def test_large_plane_forward(shape, dtype, record_property):
+    """Planes beyond shared memory (the paper's 256^2 .. 1024^2 shapes): served through the caller
+    workspace (gspn_args_t.workspace, allocated by the binding from gspn_workspace_bytes).  Whole tensor against the oracle."""
+    cfg = gi.small_config("big", *shape, seed=141)
+    B, C, H, W, G = shape
+    need = gspn.lib().gspn_workspace_bytes(B, C, H, W, G, 15, 0 if dtype == "f32" else 1, 0)
+    r = pu.check_fwd(cfg, dtype)
+    record_property("variant", r["variant"])
+    assert r["ok"], r
+    if 4 * H * W + 8 * (max(H, W) + 2) > 227 * 1024:
+        assert need == 4 * B * C * H * W
+        assert r["variant"] != "naive_fwd"                 # the shared-memory mode cannot hold it (flat_fwd takes lines up to 256)
+        if max(H, W) > 256:
+            assert r["variant"] == "naive_fwd_ws", r["variant"]
+    else:
+        assert need == 0
+
+
+@pytest.mark.parametrize("shape,dtype", [((1, 2, 160, 160, 1), "bf16"), ((1, 4, 128, 128, 1), "bf16"), ((1, 2, 256, 256, 2), "f32"),
+                                         ((1, 1, 600, 40, 1), "bf16")], ids=["160x160-bf16", "128x128-cg4-bf16", "256x256-f32", "600x40-bf16"])
+def test_large_plane_backward(shape, dtype, record_property):
+    """The backward of planes no kernel holds on chip (from about 120 x 120): every gradient against the oracle; the
+    variant that ran is recorded."""
+    cfg = gi.small_config("bigb", *shape, seed=142, backward=True)
+    r = pu.check_bwd(cfg, dtype, with_h0=True)
+    record_property("variant", r["variant"])
+    assert r["ok"], r
+
+
+def test_workspace_errors():
+    """Without a workspace the large-plane shapes report GSPN_EWORKSPACE (status 4) through the plain C call; a forced
+    fused kernel still reports GSPN_EUNSUPPORTED."""
+    import ctypes
+    cfg = gi.small_config("bige", 1, 2, 256, 256, 1, seed=143)
+    d = {k: v.cuda() for k, v in gi.make_inputs(cfg, "f32").items()}
+    y = torch.empty_like(d["x"])
+    p = lambda t: ctypes.c_void_p(t.data_ptr())
+    rc = gspn.lib().gspn_scan_fwd(p(d["x"]), p(d["w3"]), p(d["lam"]), p(d["u"]), p(y), 1, 2, 256, 256, 1, 15, 0, None)
+    assert rc == 4 and b"workspace" in gspn.lib().gspn_last_error()
+    with pytest.raises(gspn.GspnError) as ei:
+        gspn.gspn_scan_fwd(d["x"], d["w3"], d["lam"], d["u"], cfg.G, 15, impl=gspn.IMPL_CHAIN)
     assert ei.value.status == 2
