@@ -534,89 +534,96 @@ def main():
             except Exception as ex:      # noqa: BLE001
                 fused_note = {"fused_call": "raised " + repr(ex)[:200]}
         if e2e is None:
-            e2e, _ = e2e_leg(False)
+            try:
+                e2e, _ = e2e_leg(False)
+            except Exception as ex:      # noqa: BLE001 -- the device-timed line is still printed
+                e2e = {"value": None, "unit": "GB/s", "error": repr(ex)[:300]}
             if want_bwd and world == 1:
                 e2e.update(fused_note)
     del grads, y
 
     others = None
-    if not args.no_others and world == 1:
-        others = {}
-        del tensors
-        torch.cuda.empty_cache()
-        for name, oc in gi.CONFIGS.items():
-            for dt in oc.dtypes:
-                if name == cfg.name and dt == dtype:
-                    continue
-                so = 4 if dt == "f32" else 2
-                # the backward of every other config is timed too, with whatever kernel GSPN_IMPL_AUTO picks (the variant
-                # is printed: a naive fall-through shows)
-                ob = impl == gspn.IMPL_AUTO
-                try:
-                    r, tt, yy, gg = time_config(gspn, torch, oc, dt, max(5, min(steps, 20)), 3, 1, impl, ob)
-                except gspn.GspnError as ex:      # no kernel holds the backward of this shape: say so, time the forward
-                    others[f"{name}:{dt}:bwd"] = {"variant": None, "error": str(ex)[:200]}
-                    ob = False
-                    torch.cuda.empty_cache()
-                    r, tt, yy, gg = time_config(gspn, torch, oc, dt, max(5, min(steps, 20)), 3, 1, impl, ob)
-                if ob:
-                    bb = oc.bwd_bytes(so)
-                    others[f"{name}:{dt}:bwd"] = {"variant": r["variant_bwd"], "ms": r["bwd_ms_mean"], "ms_min": r["bwd_ms_min"],
-                                                   "gbs": bb / (r["bwd_ms_mean"] * 1e-3) / 1e9,
-                                                   "frac": bb / (r["bwd_ms_mean"] * 1e-3) / 1e9 / peak,
-                                                   "pxch_per_s": oc.n / (r["bwd_ms_mean"] * 1e-3), "l2_flush": r["l2_flush"]}
-                fb = oc.fwd_bytes(so)
-                others[f"{name}:{dt}:fwd"] = {"variant": r["variant_fwd"], "ms": r["fwd_ms_mean"], "ms_min": r["fwd_ms_min"],
-                                               "gbs": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9,
-                                               "frac": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9 / peak,
-                                               "pxch_per_s": oc.n / (r["fwd_ms_mean"] * 1e-3), "l2_flush": r["l2_flush"]}
-                del tt, yy, gg
-                torch.cuda.empty_cache()
-        # the fused Eq. 3 normalisation of the tap logits and its adjoint on every config
-        # (algorithmic bytes: logits read + taps written = 2 D n_w s; backward reads logits and dw3, writes dwt = 3 D n_w s)
-        for name, oc in gi.CONFIGS.items():
-            for dt in oc.dtypes:
-                so = 4 if dt == "f32" else 2
-                lg = gi.make_logits(oc, dt, device=torch.device("cuda", torch.cuda.current_device()), with_dw=True)
-                buf = torch.empty_like(lg["wt"])
-                for tag, fn, nbytes in (("norm_fwd", lambda: gspn.gspn_normalize_fwd(lg["wt"], oc.dir_mask, out=buf), 2),
-                                        ("norm_bwd", lambda: gspn.gspn_normalize_bwd(lg["wt"], lg["dw3"], oc.dir_mask, out=buf), 3)):
-                    for _ in range(3):
-                        fn()
-                    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-                    nrep = max(5, min(steps, 20))
-                    ev[0].record()
-                    for _ in range(nrep):
-                        fn()
-                    ev[1].record()
-                    torch.cuda.synchronize()
-                    ms = ev[0].elapsed_time(ev[1]) / nrep
-                    nb = nbytes * oc.D * oc.n_w * so
-                    others[f"{name}:{dt}:{tag}"] = {"variant": gspn.gspn_last_variant(), "ms": ms,
-                                                    "gbs": nb / (ms * 1e-3) / 1e9, "frac": nb / (ms * 1e-3) / 1e9 / peak}
-                del lg, buf
-                torch.cuda.empty_cache()
-
-    if others is not None and impl == gspn.IMPL_AUTO:
-        # SURVEY 8(f) f2, first step (Table 1): the paper's large planes, forward, with whatever
-        # GSPN_IMPL_AUTO picks -- today the fall-back kernels (flat_fwd up to 256 positions, beyond that the naive kernel
-        # with its accumulator plane in the workspace): correct, far from the roofline, printed so that the distance shows
-        for B_, C_, L_ in ((16, 8, 256), (16, 8, 512), (16, 8, 1024)):
-            key = f"table1:{B_}x{C_}x{L_}x{L_}:bf16:fwd"
-            try:
-                oc = gi.small_config(f"table1_{L_}", B_, C_, L_, L_, 2, seed=7)
-                r, tt, yy, gg = time_config(gspn, torch, oc, "bf16", 3, 3, 1, impl, False)
-                fb = oc.fwd_bytes(2)
-                others[key] = {"variant": r["variant_fwd"], "ms": r["fwd_ms_mean"], "ms_min": r["fwd_ms_min"],
-                               "gbs": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9, "frac": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9 / peak,
-                               "pxch_per_s": oc.n / (r["fwd_ms_mean"] * 1e-3), "l2_flush": r["l2_flush"]}
-                del tt, yy, gg
-            except Exception as ex:      # noqa: BLE001 -- a row that cannot be measured says why
-                others[key] = {"variant": None, "error": repr(ex)[:200]}
+    # whatever happens while the other configs are timed, the main line above is already measured and must be printed
+    try:
+        if not args.no_others and world == 1:
+            others = {}
+            del tensors
             torch.cuda.empty_cache()
+            for name, oc in gi.CONFIGS.items():
+                for dt in oc.dtypes:
+                    if name == cfg.name and dt == dtype:
+                        continue
+                    so = 4 if dt == "f32" else 2
+                    # the backward of every other config is timed too, with whatever kernel GSPN_IMPL_AUTO picks (the variant
+                    # is printed: a naive fall-through shows)
+                    ob = impl == gspn.IMPL_AUTO
+                    try:
+                        r, tt, yy, gg = time_config(gspn, torch, oc, dt, max(5, min(steps, 20)), 3, 1, impl, ob)
+                    except gspn.GspnError as ex:      # no kernel holds the backward of this shape: say so, time the forward
+                        others[f"{name}:{dt}:bwd"] = {"variant": None, "error": str(ex)[:200]}
+                        ob = False
+                        torch.cuda.empty_cache()
+                        r, tt, yy, gg = time_config(gspn, torch, oc, dt, max(5, min(steps, 20)), 3, 1, impl, ob)
+                    if ob:
+                        bb = oc.bwd_bytes(so)
+                        others[f"{name}:{dt}:bwd"] = {"variant": r["variant_bwd"], "ms": r["bwd_ms_mean"], "ms_min": r["bwd_ms_min"],
+                                                       "gbs": bb / (r["bwd_ms_mean"] * 1e-3) / 1e9,
+                                                       "frac": bb / (r["bwd_ms_mean"] * 1e-3) / 1e9 / peak,
+                                                       "pxch_per_s": oc.n / (r["bwd_ms_mean"] * 1e-3), "l2_flush": r["l2_flush"]}
+                    fb = oc.fwd_bytes(so)
+                    others[f"{name}:{dt}:fwd"] = {"variant": r["variant_fwd"], "ms": r["fwd_ms_mean"], "ms_min": r["fwd_ms_min"],
+                                                   "gbs": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9,
+                                                   "frac": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9 / peak,
+                                                   "pxch_per_s": oc.n / (r["fwd_ms_mean"] * 1e-3), "l2_flush": r["l2_flush"]}
+                    del tt, yy, gg
+                    torch.cuda.empty_cache()
+            # the fused Eq. 3 normalisation of the tap logits and its adjoint on every config
+            # (algorithmic bytes: logits read + taps written = 2 D n_w s; backward reads logits and dw3, writes dwt = 3 D n_w s)
+            for name, oc in gi.CONFIGS.items():
+                for dt in oc.dtypes:
+                    so = 4 if dt == "f32" else 2
+                    lg = gi.make_logits(oc, dt, device=torch.device("cuda", torch.cuda.current_device()), with_dw=True)
+                    buf = torch.empty_like(lg["wt"])
+                    for tag, fn, nbytes in (("norm_fwd", lambda: gspn.gspn_normalize_fwd(lg["wt"], oc.dir_mask, out=buf), 2),
+                                            ("norm_bwd", lambda: gspn.gspn_normalize_bwd(lg["wt"], lg["dw3"], oc.dir_mask, out=buf), 3)):
+                        for _ in range(3):
+                            fn()
+                        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+                        nrep = max(5, min(steps, 20))
+                        ev[0].record()
+                        for _ in range(nrep):
+                            fn()
+                        ev[1].record()
+                        torch.cuda.synchronize()
+                        ms = ev[0].elapsed_time(ev[1]) / nrep
+                        nb = nbytes * oc.D * oc.n_w * so
+                        others[f"{name}:{dt}:{tag}"] = {"variant": gspn.gspn_last_variant(), "ms": ms,
+                                                        "gbs": nb / (ms * 1e-3) / 1e9, "frac": nb / (ms * 1e-3) / 1e9 / peak}
+                    del lg, buf
+                    torch.cuda.empty_cache()
 
-    if others is not None and impl == gspn.IMPL_AUTO and not args.no_line_bwd_probe:
-        others["line_bwd_child"] = line_bwd_probe()
+        if others is not None and impl == gspn.IMPL_AUTO:
+            # SURVEY 8(f) f2, first step (Table 1): the paper's large planes, forward, with whatever
+            # GSPN_IMPL_AUTO picks -- today the fall-back kernels (flat_fwd up to 256 positions, beyond that the naive kernel
+            # with its accumulator plane in the workspace): correct, far from the roofline, printed so that the distance shows
+            for B_, C_, L_ in ((16, 8, 256), (16, 8, 512), (16, 8, 1024)):
+                key = f"table1:{B_}x{C_}x{L_}x{L_}:bf16:fwd"
+                try:
+                    oc = gi.small_config(f"table1_{L_}", B_, C_, L_, L_, 2, seed=7)
+                    r, tt, yy, gg = time_config(gspn, torch, oc, "bf16", 3, 3, 1, impl, False)
+                    fb = oc.fwd_bytes(2)
+                    others[key] = {"variant": r["variant_fwd"], "ms": r["fwd_ms_mean"], "ms_min": r["fwd_ms_min"],
+                                   "gbs": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9, "frac": fb / (r["fwd_ms_mean"] * 1e-3) / 1e9 / peak,
+                                   "pxch_per_s": oc.n / (r["fwd_ms_mean"] * 1e-3), "l2_flush": r["l2_flush"]}
+                    del tt, yy, gg
+                except Exception as ex:      # noqa: BLE001 -- a row that cannot be measured says why
+                    others[key] = {"variant": None, "error": repr(ex)[:200]}
+                torch.cuda.empty_cache()
+
+        if others is not None and impl == gspn.IMPL_AUTO and not args.no_line_bwd_probe:
+            others["line_bwd_child"] = line_bwd_probe()
+    except Exception as ex:      # noqa: BLE001
+        others = dict(others or {}, error="others aborted: " + repr(ex)[:300])
 
     cpu = None
     if not args.no_cpu and rank == 0 and world == 1:
