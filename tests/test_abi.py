@@ -150,6 +150,17 @@ def test_dir_stride_fields_are_validated_without_gpu(L):
     # flags: GSPN_FLAG_W3_LOGITS accepted, unknown bits refused
     assert call(flags=1) == 0
     assert call(flags=2) == 1 and b"flags" in L.gspn_last_error()
+    # the options the naive kernels alone serve are refused by a forced fused kernel before anything is launched
+    def fwd_forced(**kw):
+        a = bd._Args(struct_size=ctypes.sizeof(bd._Args), x=p, w3=p, lam=p, u=p, y=p, B=B, C=C, H=H, W=W, G=G, dir_mask=15, dtype=0,
+                     impl=gspn.IMPL_CHAIN, dir_stride_w3=bd.DIR_STRIDE_DENSE, dir_stride_lambda=bd.DIR_STRIDE_DENSE,
+                     dir_stride_u=bd.DIR_STRIDE_DENSE)
+        for k, v in kw.items():
+            setattr(a, k, v)
+        return L.gspn_scan_fwd_ex(ctypes.byref(a))
+    assert fwd_forced(dir_stride_w3=0) == 2 and b"naive kernels only" in L.gspn_last_error()
+    assert fwd_forced(k_chunk=3) == 2 and fwd_forced(flags=1) == 2
+    assert fwd_forced(workspace=p + 8) == 3 and b"workspace" in L.gspn_last_error()
     # the binding's helper: names -> strides
     assert bd._strides(("w3",)) == {"dir_stride_w3": 0, "dir_stride_lambda": bd.DIR_STRIDE_DENSE, "dir_stride_u": bd.DIR_STRIDE_DENSE}
     with pytest.raises(ValueError):
