@@ -19,6 +19,7 @@ namespace gspn {
 constexpr int kBlk = 4;            // scan steps per block = checkpoint interval = ring stage (lines / chunk columns)
 constexpr int kChSlots = 8;        // mbarrier pairs (ring slots) available
 
+#ifndef GSPN_EMU      // (tests/emu/emu_ptx.h stands in for Elem, cp_async_cb, l2_prefetch_bulk, chain_bar, lds32, sts32)
 template <typename ST> struct Elem;
 template <> struct Elem<__nv_bfloat16> {
     using raw_t = unsigned short;
@@ -71,6 +72,7 @@ template <> __device__ __forceinline__ void cp_async_cb<16>(uint32_t dst, const 
 __device__ __forceinline__ void l2_prefetch_bulk(const void* p, uint32_t bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
+#endif  // GSPN_EMU
 // prefetch the 16-byte-aligned superset of plane e (HWB bytes long) that lies inside its tensor
 __device__ __forceinline__ void l2_prefetch_plane(const uint8_t* base, unsigned long long b0, unsigned long long tbytes,
                                                   unsigned long long HWB) {
@@ -82,9 +84,7 @@ __device__ __forceinline__ void l2_prefetch_plane(const uint8_t* base, unsigned 
 }
 
 // named barrier among the chain warps of a CTA (the producer warp does not take part)
-__device__ __forceinline__ void chain_bar(int nthreads) {
-    asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
-}
+__device__ __forceinline__ void chain_bar(int nthreads) { named_bar_sync(1, nthreads); }
 
 struct ChPlane {                  // one operand plane of one direction (table in shared memory)
     const uint8_t* base;          // tensor base (16-byte aligned)
@@ -93,12 +93,14 @@ struct ChPlane {                  // one operand plane of one direction (table i
 };
 
 __device__ __forceinline__ float maskf(float v, uint32_t m) { return __uint_as_float(__float_as_uint(v) & m); }
+#ifndef GSPN_EMU
 __device__ __forceinline__ float lds32(uint32_t a) {
     float v;
     asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
     return v;
 }
 __device__ __forceinline__ void sts32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v)); }
+#endif
 
 // ---------------------------------------------------------------------------------------------------
 // Ring hand-shake of a consumer warp.  Block bi (image lines [4bi, 4bi+4)) needs row block bi

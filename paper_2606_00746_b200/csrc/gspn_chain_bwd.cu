@@ -216,7 +216,7 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
         }
     }
     // the checkpoints written by ROLE_A are read by ROLE_F of the same channel
-    asm volatile("bar.sync %0, 64;" ::"r"(2 + c) : "memory");
+    named_bar_sync(2 + c, 64);
 
     // ================= pass 2: reverse order ===========================================================
     constexpr bool desc2 = !REV;
@@ -298,7 +298,7 @@ __device__ __forceinline__ void chain_bwd_dir(const ChainBwdParams& p, uint8_t* 
         }
     }
     // ROLE_A must not overwrite the checkpoints (next direction) while ROLE_F still reads them
-    asm volatile("bar.sync %0, 64;" ::"r"(2 + c) : "memory");
+    named_bar_sync(2 + c, 64);
     pf = rs.pf;
 }
 
@@ -469,7 +469,7 @@ __device__ __forceinline__ void chain_bwd_out(const ChainBwdParams& p, uint8_t* 
         if constexpr (VH) {
             const bool pair_done = desc2 ? ((bi & 1) == 0) : ((bi & 1) == 1 || bi == NB - 1);
             if (pair_done) {
-                asm volatile("bar.sync 10, 128;" ::: "memory");
+                named_bar_sync(10, 128);
                 const int col0 = 2 * kBlk * (bi >> 1);
                 const int ncols = min(2 * kBlk, W - col0);
                 const int col = lane & 7, rsub = lane >> 3;
@@ -489,7 +489,7 @@ __device__ __forceinline__ void chain_bwd_out(const ChainBwdParams& p, uint8_t* 
                         }
                     }
                 }
-                asm volatile("bar.sync 10, 128;" ::: "memory");
+                named_bar_sync(10, 128);
             }
         }
         rs.release(bi, desc2, n == NB - 1);
@@ -545,7 +545,7 @@ chain_bwd_kernel(const ChainBwdParams p) {
         for (int s = 0; s < 2; ++s) { mbar_init(&empty[kChSlots + s], 2 * NS); mbar_init(&empty[kChSlots + 2 + s], kChNO); }
         mbar_init_fence();
     }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // zeros (generic proxy) before bulk copies
+    fence_proxy_async();      // zeros (generic proxy) before bulk copies
     __syncthreads();
 
     if (warp < kChNPW) {
@@ -738,7 +738,7 @@ static int launch_chain_bwd(const ChainBwdParams& prm, int items, int threads, c
     auto kern = chain_bwd_kernel<ST, P>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("chain bwd: cudaFuncSetAttribute(%u B): %s", prm.total, cudaGetErrorString(e)); return GSPN_ECUDA; }
-    kern<<<items, threads, prm.total, st>>>(prm);
+    GSPN_LAUNCH(kern, items, threads, prm.total, st, prm);
     e = cudaGetLastError();
     if (e != cudaSuccess) { set_error("chain bwd: launch failed: %s", cudaGetErrorString(e)); return GSPN_ECUDA; }
     return GSPN_OK;

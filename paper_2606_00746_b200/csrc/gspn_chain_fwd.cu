@@ -220,7 +220,7 @@ chain_fwd_kernel(const ChainFwdParams p) {
         for (int s = 0; s < kChSlots; ++s) { mbar_init(&full[s], kCfNPW * 33); mbar_init(&empty[s], NC); }
         mbar_init_fence();
     }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // zeros (generic proxy) before bulk copies
+    fence_proxy_async();      // zeros (generic proxy) before bulk copies
     __syncthreads();
 
     if (warp < kCfNPW) {
@@ -379,7 +379,7 @@ static int launch_chain_fwd(const ChainFwdParams& prm, int items, int threads, c
     auto kern = chain_fwd_kernel<ST, P, CBH>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("chain fwd: cudaFuncSetAttribute(%u B): %s", prm.total, cudaGetErrorString(e)); return GSPN_ECUDA; }
-    kern<<<items, threads, prm.total, st>>>(prm);
+    GSPN_LAUNCH(kern, items, threads, prm.total, st, prm);
     e = cudaGetLastError();
     if (e != cudaSuccess) { set_error("chain fwd: launch failed: %s", cudaGetErrorString(e)); return GSPN_ECUDA; }
     return GSPN_OK;

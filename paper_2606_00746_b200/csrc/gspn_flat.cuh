@@ -25,6 +25,7 @@
 
 namespace gspn {
 
+#ifndef GSPN_EMU      // (tests/emu/emu_ptx.h stands in for the PTX wrappers, see gspn_fused.cuh)
 // 16-byte cp.async (LDGSTS) global -> shared
 __device__ __forceinline__ void cp_async_16(void* dst, const void* src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
@@ -54,6 +55,7 @@ __device__ __forceinline__ float lds_f32(uint32_t addr) {
 __device__ __forceinline__ void sts_f32(uint32_t addr, float v) {
     asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
 }
+#endif  // GSPN_EMU
 
 __device__ __forceinline__ int warp_sum(int v) {
 #pragma unroll

@@ -79,6 +79,12 @@ __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* m) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(m) : "memory");
 }
+// named barrier `id` (1..15) among `nthreads` threads (whole warps) of the CTA
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+// generic-proxy writes to shared memory are ordered before later async-proxy (bulk / TMA) accesses
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 #endif  // GSPN_EMU
 
 // ---- storage vectors ---------------------------------------------------------------------------

@@ -65,10 +65,6 @@ __device__ __forceinline__ void mbar_wait_spin(uint64_t* b, uint32_t parity) {
         "}\n" ::"r"(smem_u32(b)), "r"(parity) : "memory");
 }
 
-__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-
 // ---- tensor memory (TMEM) as the fp32 accumulator store ----------------------------------------------------------
 // 128 lanes x 512 columns x 32 bit per SM; warp w of a CTA reaches lanes 32*(w % 4) .. +31, one lane per thread
 // (shape 32x32b: thread t reads / writes N consecutive columns of its own lane).  Addresses: lane << 16 | column.
@@ -150,7 +146,6 @@ template <int N> __device__ __forceinline__ void bulk_wait_read() {
 template <int N> __device__ __forceinline__ void bulk_wait_all() {
     asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory");
 }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 __device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* m, int c0, int c1, int c2, int c3, int c4,
                                             uint64_t* bar) {

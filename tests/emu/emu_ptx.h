@@ -175,6 +175,56 @@ inline void tm_wait_st() {}
 inline void tm_fence_before() {}
 inline void tm_fence_after() {}
 
+// ---- csrc/gspn_flat.cuh / gspn_chain.cuh: shared memory addressed by 32-bit shared-window addresses, cp.async ----------------
+// smem_u32() above hands out offsets from the start of the CTA's shared memory; these turn them back into pointers.
+template <typename T> inline T* emu_sptr(uint32_t a, const char* what) {
+    unsigned char* p = const_cast<unsigned char*>(emu::smem_lo) + a;
+    emu::check_smem(p, sizeof(T), what);
+    if ((uintptr_t)p % sizeof(T)) emu::fail("%s: shared address %u is not %zu-byte aligned", what, a, sizeof(T));
+    return reinterpret_cast<T*>(p);
+}
+inline float lds_f32(uint32_t a) { return *emu_sptr<float>(a, "ld.shared.f32"); }
+inline void sts_f32(uint32_t a, float v) { *emu_sptr<float>(a, "st.shared.f32") = v; }
+inline float lds32(uint32_t a) { return lds_f32(a); }
+inline void sts32(uint32_t a, float v) { sts_f32(a, v); }
+template <typename ST> inline float lds_f(uint32_t a);
+template <> inline float lds_f<float>(uint32_t a) { return lds_f32(a); }
+template <> inline float lds_f<__nv_bfloat16>(uint32_t a) { return __uint_as_float(((uint32_t)*emu_sptr<unsigned short>(a, "ld.shared.u16")) << 16); }
+// cp.async: the copy happens at once; cp.async.mbarrier.arrive.noinc is then a plain arrival (the count was pre-armed)
+inline void emu_cp_async(void* dst, const void* src, int bytes) {
+    if (((uintptr_t)dst | (uintptr_t)src) % bytes) emu::fail("cp.async: %d-byte copy with an unaligned address (shared offset %ld)", bytes, emu::smem_off(dst));
+    emu::check_smem(dst, bytes, "cp.async");
+    std::memcpy(dst, src, bytes);
+}
+inline void cp_async_16(void* dst, const void* src) { emu_cp_async(dst, src, 16); }
+inline void cp_async_arrive_noinc(uint64_t* bar) { emu::mb_arrive(bar, 0); }
+template <int CB> inline void cp_async_cb(uint32_t dst, const void* src) {
+    static_assert(CB == 8 || CB == 16, "cp_async_cb");
+    emu_cp_async(const_cast<unsigned char*>(emu::smem_lo) + dst, src, CB);
+}
+inline void l2_prefetch_bulk(const void* p, uint32_t bytes) {
+    if (((uintptr_t)p & 15u) || (bytes & 15u) || bytes == 0) emu::fail("cp.async.bulk.prefetch.L2: address or size %u not a multiple of 16", bytes);
+}
+template <typename ST> struct Elem;
+template <> struct Elem<__nv_bfloat16> {
+    using raw_t = unsigned short;
+    static raw_t lds(uint32_t a) { return *emu_sptr<raw_t>(a, "ld.shared.u16"); }
+    static void sts(uint32_t a, raw_t v) { *emu_sptr<raw_t>(a, "st.shared.u16") = v; }
+    static float f(raw_t r) { return __uint_as_float(((uint32_t)r) << 16); }
+    static float fma2(raw_t a, raw_t b, float c) { return fmaf(f(a), f(b), c); }
+    static raw_t pack(float v) { return __bfloat16_as_ushort(__float2bfloat16_rn(v)); }
+    static void stg(__nv_bfloat16* p, raw_t v) { *reinterpret_cast<raw_t*>(p) = v; }
+};
+template <> struct Elem<float> {
+    using raw_t = float;
+    static raw_t lds(uint32_t a) { return lds_f32(a); }
+    static void sts(uint32_t a, raw_t v) { sts_f32(a, v); }
+    static float f(raw_t r) { return r; }
+    static float fma2(raw_t a, raw_t b, float c) { return fmaf(a, b, c); }
+    static raw_t pack(float v) { return v; }
+    static void stg(float* p, raw_t v) { *p = v; }
+};
+
 // fma.rn.f32.bf16: c + a * b with a, b the low or high bf16 half of a 32-bit word, one rounding
 inline float fma_bf16_half(uint32_t a, uint32_t b, bool high, float c) {
     const float fa = __uint_as_float(high ? (a & 0xffff0000u) : (a << 16)), fb = __uint_as_float(high ? (b & 0xffff0000u) : (b << 16));
