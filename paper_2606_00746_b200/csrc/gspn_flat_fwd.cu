@@ -458,7 +458,7 @@ static int launch_flat(const FlatPlan& pl, int items, cudaStream_t st) {
     auto kern = fwd_flat_kernel<ST, P, CS>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("flat fwd: cudaFuncSetAttribute(%zu B): %s", pl.smem, cudaGetErrorString(e)); return GSPN_ECUDA; }
-    kern<<<items, pl.threads, pl.smem, st>>>(pl.prm);
+    GSPN_LAUNCH(kern, items, pl.threads, pl.smem, st, pl.prm);
     e = cudaGetLastError();
     if (e != cudaSuccess) { set_error("flat fwd: launch failed: %s", cudaGetErrorString(e)); return GSPN_ECUDA; }
     return GSPN_OK;

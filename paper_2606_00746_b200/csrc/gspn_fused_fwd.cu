@@ -407,7 +407,7 @@ static int launch_tile(const FwdArgs<ST>& a, const TilePlan& pl, cudaStream_t st
     if (e != cudaSuccess) { set_error("fused fwd: cudaFuncSetAttribute(%zu B): %s", pl.smem, cudaGetErrorString(e)); return GSPN_ECUDA; }
     const int items = sh.B * sh.G * (sh.cg() / cpc);
     const int threads = (4 + 4 * cpc) * 32;
-    kern<<<items, threads, pl.smem, st>>>(m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], pl.prm);
+    GSPN_LAUNCH(kern, items, threads, pl.smem, st, m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], pl.prm);
     e = cudaGetLastError();
     if (e != cudaSuccess) { set_error("fused fwd: launch failed: %s", cudaGetErrorString(e)); return GSPN_ECUDA; }
     return GSPN_OK;

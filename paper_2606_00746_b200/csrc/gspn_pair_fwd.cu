@@ -70,8 +70,8 @@ template <> struct PfTap<float> {
 // named barrier of the two warps of an axis and channel set (ids 1.. vertical, 8.. horizontal: the axes of the
 // whole-plane kernel run at the same time)
 template <bool SECOND = false> __device__ __forceinline__ void pf_pair_bar(int set = 0) {
-    if constexpr (SECOND) asm volatile("bar.sync %0, 64;" ::"r"(8 + set) : "memory");
-    else asm volatile("bar.sync %0, 64;" ::"r"(1 + set) : "memory");
+    if constexpr (SECOND) named_bar_sync(8 + set, 64);
+    else named_bar_sync(1 + set, 64);
 }
 
 // One direction, all NC channels of the CTA, on one warp.  VH = false: T->B / B->T (lanes own columns), true:
@@ -410,7 +410,7 @@ static int launch_plane_fwd(const PairFwdParams& prm, int items, cudaStream_t st
     auto kern = plane_fwd_kernel<ST, P, NC, NCW>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("plane fwd: cudaFuncSetAttribute(%u B): %s", prm.total, cudaGetErrorString(e)); return GSPN_ECUDA; }
-    kern<<<items, 32 * (4 * (NC / NCW) + 1), prm.total, st>>>(prm);
+    GSPN_LAUNCH(kern, items, 32 * (4 * (NC / NCW) + 1), prm.total, st, prm);
     e = cudaGetLastError();
     if (e != cudaSuccess) { set_error("plane fwd: launch failed: %s", cudaGetErrorString(e)); return GSPN_ECUDA; }
     return GSPN_OK;

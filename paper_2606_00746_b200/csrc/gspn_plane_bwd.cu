@@ -147,7 +147,7 @@ __device__ __forceinline__ void plane_bwd_dir(const PlaneBwdParams& p, uint8_t* 
     }
     __syncwarp();
     if constexpr (PART != 0) {
-        asm volatile("bar.sync %0, 64;" ::"r"(3 + d) : "memory");      // both halves of h are in shared memory
+        named_bar_sync(3 + d, 64);      // both halves of h are in shared memory
         if constexpr (PART == 2) return;
     }
 
@@ -161,7 +161,7 @@ __device__ __forceinline__ void plane_bwd_dir(const PlaneBwdParams& p, uint8_t* 
     for (int s = Ls - 1; s >= 0; --s) {
         const int li = REV ? Ls - 1 - s : s;                             // image line of this step
         // REV walks the lines upwards in pass 2, !REV downwards: the downward warp waits before line `mid`
-        if (!REV && pair_sync && li == mid) asm volatile("bar.sync %0, 64;" ::"r"(VH ? 2 : 1) : "memory");
+        if (!REV && pair_sync && li == mid) named_bar_sync(VH ? 2 : 1, 64);
         const uint32_t lo = (uint32_t)li * step;
         const float w0 = E::f(E::lds(A[0] + lo)), w1 = E::f(E::lds(A[1] + lo)), w2 = E::f(E::lds(A[2] + lo));
         float dw0 = 0.f, dw1 = 0.f, dw2 = 0.f;
@@ -191,7 +191,7 @@ __device__ __forceinline__ void plane_bwd_dir(const PlaneBwdParams& p, uint8_t* 
             E::sts(A[1] + lo, E::pack(dw1));
             E::sts(A[2] + lo, E::pack(dw2));
         }
-        if (REV && pair_sync && li == mid) asm volatile("bar.sync %0, 64;" ::"r"(VH ? 2 : 1) : "memory");
+        if (REV && pair_sync && li == mid) named_bar_sync(VH ? 2 : 1, 64);
     }
     if (p.dh0 && lane < Lmax) {                                    // entries past the line are zeros
 #pragma unroll
@@ -267,7 +267,7 @@ plane_bwd_kernel(const PlaneBwdParams p) {
             if (warp == 6 && act[2]) plane_bwd_dir<ST, NC, true, false, 2>(p, smem, 2, b, g, lane, act[3]);
             if (warp == 7 && act[3]) plane_bwd_dir<ST, NC, true, true, 2>(p, smem, 3, b, g, lane, act[2]);
         }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // the in-place outputs, before the bulk stores read them
+        fence_proxy_async();    // the in-place outputs, before the bulk stores read them
     }
     __syncthreads();
 
@@ -300,16 +300,15 @@ plane_bwd_kernel(const PlaneBwdParams p) {
         const uint8_t* src = smem + p.off_pl + (size_t)pl * p.plslot + phase;
         uint8_t* dst = reinterpret_cast<uint8_t*>(out) + b0;
         if (lane == 0 && inner > 0)
-            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst + head),
-                         "r"(smem_u32(src + head)), "r"(inner) : "memory");
+            bulk_store_1d(dst + head, src + head, inner);
         for (uint32_t o = lane * ES; o < head; o += 32 * ES)
             *reinterpret_cast<ST*>(dst + o) = *reinterpret_cast<const ST*>(src + o);
         for (uint32_t o = head + inner + lane * ES; o < hwb; o += 32 * ES)
             *reinterpret_cast<ST*>(dst + o) = *reinterpret_cast<const ST*>(src + o);
     }
     // shared memory must outlive the bulk stores' reads
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    bulk_commit();
+    bulk_wait_read<0>();
 }
 
 // ---- host side -----------------------------------------------------------------------------------
@@ -340,7 +339,7 @@ static int launch_plane_bwd(const PlaneBwdParams& prm, int items, cudaStream_t s
     auto kern = plane_bwd_kernel<ST, NC>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemOptin);
     if (e != cudaSuccess) { set_error("plane bwd: cudaFuncSetAttribute(%u B): %s", prm.total, cudaGetErrorString(e)); return GSPN_ECUDA; }
-    kern<<<items, NC >= 2 ? 288 : 160, prm.total, st>>>(prm);
+    GSPN_LAUNCH(kern, items, NC >= 2 ? 288 : 160, prm.total, st, prm);
     e = cudaGetLastError();
     if (e != cudaSuccess) { set_error("plane bwd: launch failed: %s", cudaGetErrorString(e)); return GSPN_ECUDA; }
     return GSPN_OK;

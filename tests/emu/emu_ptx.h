@@ -132,6 +132,13 @@ inline void bulk_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* b
     emu::check_smem(dst, bytes, "cp.async.bulk");
     emu_issue_load(bar, [=]() -> long long { std::memcpy(dst, src, bytes); return (long long)bytes; });
 }
+inline void bulk_store_1d(void* dst, const void* src, uint32_t bytes) {
+    if (((uintptr_t)dst & 15u) || ((uintptr_t)src & 15u) || (bytes & 15u))
+        emu::fail("cp.async.bulk (store): source (shared offset %ld), destination or size %u not 16-byte aligned", emu::smem_off(src), bytes);
+    emu::check_smem(src, bytes, "cp.async.bulk (store)");
+    if (!emu::lazy) { std::memcpy(dst, src, bytes); return; }
+    emu::store_open.emplace_back([=] { std::memcpy(dst, src, bytes); });
+}
 inline void tma_prefetch_desc(const CUtensorMap* m) { (void)emu_map(m); }
 
 // ---- tensor memory: shape 32x32b, thread t of a warp reaches lane 32 * (warp % 4) + t only ------------------------------------

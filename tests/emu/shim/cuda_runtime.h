@@ -44,6 +44,19 @@ inline uint32_t __float_as_uint(float f) { uint32_t v; std::memcpy(&v, &f, 4); r
 template <typename T> inline T min(T a, T b) { return b < a ? b : a; }      // CUDA declares these at global scope
 template <typename T> inline T max(T a, T b) { return a < b ? b : a; }
 
+// PRMT: byte i of the result is byte (selector nibble i & 7) of {y:x}; nibble bit 3 replicates that byte's sign bit
+inline unsigned __byte_perm(unsigned x, unsigned y, unsigned s) {
+    const unsigned long long v = ((unsigned long long)y << 32) | x;
+    unsigned r = 0;
+    for (int i = 0; i < 4; ++i) {
+        const unsigned sel = (s >> (4 * i)) & 0xfu;
+        unsigned b = (unsigned)(v >> (8 * (sel & 7u))) & 0xffu;
+        if (sel & 8u) b = (b & 0x80u) ? 0xffu : 0u;
+        r |= b << (8 * i);
+    }
+    return r;
+}
+
 // warp shuffles, full mask only (every lane of the warp must execute them, as the hardware requires for the mask)
 template <typename T> inline T emu_shfl(unsigned mask, T v, int src) {
     static_assert(sizeof(T) == 4, "shuffle of 32-bit values");
