@@ -46,9 +46,11 @@
  * last non-OK status on the calling thread.
  *     GSPN_EINVAL        bad shape (B,C,H,W,G < 1, C % G != 0), dir_mask not in
  *                        [1,15], unknown dtype, NULL required pointer
- *     GSPN_EUNSUPPORTED  shape outside what the kernels hold on chip (a plane's
- *                        fp32 accumulator must fit one SM's shared memory;
- *                        max(H,W) <= 1024)
+ *     GSPN_EUNSUPPORTED  a line longer than 1024 positions (max(H,W) > 1024); a forced
+ *                        kernel (gspn_args_t.impl) that does not hold the shape or option
+ *     GSPN_EWORKSPACE    a plane whose fp32 accumulators exceed one SM's shared memory
+ *                        needs gspn_args_t.workspace (gspn_workspace_bytes), which is
+ *                        missing or too small; the plain calls pass none
  *     GSPN_EALIGN        a base pointer is not 16-byte aligned
  *     GSPN_ECUDA         a CUDA runtime call or launch failed
  * There is no CPU fallback: without a CUDA device every compute entry point
