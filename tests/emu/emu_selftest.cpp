@@ -46,9 +46,10 @@ extern "C" int st_mbar_tx() {
     return run(32, [] {
         uint64_t* b = reinterpret_cast<uint64_t*>(smem);
         static float src[64];
+        if (threadIdx.x == 0) gspn::mbar_init(b, 1);
+        __syncthreads();                                         // as in the kernels: nobody touches a barrier before its init
         if (threadIdx.x == 0) {
             for (int i = 0; i < 64; ++i) src[i] = (float)i;
-            gspn::mbar_init(b, 1);
             gspn::mbar_arrive_expect_tx(b, 256);
             gspn::bulk_load_1d(smem + 1024, src, 128, b);
             out[0] = 0;                                          // half the bytes: not complete (checked by the waiter below)
@@ -86,6 +87,9 @@ extern "C" int st_tma_clip(float* tensor) {
             const uint32_t box[3] = {8, 4, 1};
             out[0] = gspn::encode_tensor_map(&m, 4, tensor, 3, dims, strides, box) ? 1 : 0;
             gspn::mbar_init(b, 1);
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
             gspn::mbar_arrive_expect_tx(b, 8 * 4 * 4);
             gspn::tma_load_3d(smem + 1024, &m, 0, 3, 1, b);
         }
@@ -110,6 +114,9 @@ extern "C" int st_tma_swizzle(unsigned short* tensor) {
             const uint32_t box[3] = {16, 16, 1};
             out[0] = gspn::encode_tensor_map(&m, 2, tensor, 3, dims, strides, box, 1) ? 1 : 0;
             gspn::mbar_init(b, 1);
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
             gspn::mbar_arrive_expect_tx(b, 512);
             gspn::tma_load_3d(smem + 1024, &m, 0, 0, 0, b);
         }
