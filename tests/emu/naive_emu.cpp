@@ -9,7 +9,7 @@
 #include "gspn_naive.cuh"
 
 namespace gspn {
-alignas(16) float smem[1 << 20];      // dynamic shared memory of the running block (4 MB: far above the 227 KB a real CTA has)
+alignas(16) float smem[1 << 16];      // dynamic shared memory of the running block (256 KB; a real CTA has 227 KB)
 }
 
 template <typename F>

@@ -14,7 +14,7 @@ import pytest
 
 import gspn_inputs as gi
 import parity_util as pu
-from test_line_emulated_cpu import to_dev, from_dev, ptr
+from test_line_emulated_cpu import to_dev, from_dev, ptr, heavy
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 EMU = os.path.join(HERE, "emu")
@@ -53,8 +53,9 @@ def run_bwd(L, cfg, dtype, t, need=("dx", "dlambda", "du", "dw3", "dh0")):
 GROUP_SHAPES = [(1, 4, 27, 27, 1), (2, 4, 8, 8, 2), (1, 2, 40, 44, 2), (1, 4, 33, 35, 1), (1, 2, 100, 36, 1)]      # as the GPU test
 
 
-@pytest.mark.parametrize("dtype", ["f32", "bf16"])
-@pytest.mark.parametrize("shape", GROUP_SHAPES, ids=["x".join(map(str, s)) for s in GROUP_SHAPES])
+@pytest.mark.parametrize("dtype", ["f32", pytest.param("bf16", marks=heavy)])
+@pytest.mark.parametrize("shape", [pytest.param(s, marks=heavy) if max(s[2], s[3]) > 64 else s for s in GROUP_SHAPES],
+                         ids=["x".join(map(str, s)) for s in GROUP_SHAPES])
 def test_group_backward_emulated(emu, shape, dtype):
     ran = 0
     for mask in (15, 6, 9):

@@ -117,7 +117,7 @@ def _id(c):
     return "x".join(map(str, c[0])) + f"-m{c[1]}-{c[2]}" + ("-h0" if c[3] else "")
 
 
-@pytest.mark.parametrize("case", FWD_CASES, ids=[_id(c) for c in FWD_CASES])
+@pytest.mark.parametrize("case", [pytest.param(c, marks=heavy) if max(c[0][2], c[0][3]) > 64 else c for c in FWD_CASES], ids=[_id(c) for c in FWD_CASES])
 def test_line_forward_emulated(emu, case):
     shape, mask, dtype, h0 = case
     cfg = gi.small_config("lfe", *shape, dir_mask=mask, seed=7)

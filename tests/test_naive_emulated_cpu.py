@@ -22,6 +22,9 @@ import gspn_inputs as gi
 import parity_util as pu
 from oracle import gspn_oracle as orc
 
+# the default run keeps one storage type / one chunk count per option; GSPN_EMU_FULL=1 runs the full grid
+heavy = pytest.mark.skipif(os.environ.get("GSPN_EMU_FULL") != "1", reason="set GSPN_EMU_FULL=1 for the full grid of emulated cases")
+
 HERE = os.path.dirname(os.path.abspath(__file__))
 EMU = os.path.join(HERE, "emu")
 CSRC = os.path.join(os.path.dirname(HERE), "paper_2606_00746_b200", "csrc")
@@ -116,7 +119,7 @@ def test_naive_kernels_emulated_match_the_oracle(emu, shape, mask, dtype):
 SHARED_SETS = [("w3",), ("lam", "u"), ("w3", "lam", "u")]
 
 
-@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("dtype", ["f32", pytest.param("bf16", marks=heavy)])
 @pytest.mark.parametrize("shared", SHARED_SETS, ids=["+".join(s) for s in SHARED_SETS])
 def test_shared_direction_slabs_emulated(emu, shared, dtype):
     """dir_stride_* = 0: one slab read by every direction == the dense operator on the slab replicated D times."""
@@ -141,7 +144,7 @@ def test_shared_direction_slabs_emulated(emu, shared, dtype):
 
 
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
-@pytest.mark.parametrize("k_chunk", [2, 3, 7])
+@pytest.mark.parametrize("k_chunk", [pytest.param(2, marks=heavy), 3, pytest.param(7, marks=heavy)])
 def test_chunked_scan_emulated(emu, k_chunk, dtype):
     """k_chunk > 1 against oracle fwd_chunked / bwd_chunked, with h0, ragged bands and direction subsets."""
     for shape, mask in [((2, 4, 8, 8, 2), 15), ((1, 2, 13, 17, 1), 15), ((1, 2, 10, 9, 2), 6), ((1, 2, 11, 20, 1), 9)]:
